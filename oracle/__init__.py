@@ -1,0 +1,148 @@
+"""CPU oracle for the active-dumbbell hot path of arXiv 1004.1932.
+
+TEST INFRASTRUCTURE, NOT THE PRODUCT: only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this package.  The arithmetic lives in
+oracle/ds_oracle.c (plain C, fp64, scalar loops, each function citing the paper); this file
+is the ctypes marshalling around it and holds none of the method's arithmetic.  It imports
+nothing from paper_1004_1932_b200.
+"""
+import ctypes
+from dataclasses import dataclass
+
+import numpy as np
+
+from . import build as _build
+
+OSEEN, RPY = 0, 1
+EULER, HEUN = 0, 1
+
+
+class _CParams(ctypes.Structure):
+    _fields_ = [("a", ctypes.c_double), ("eta", ctypes.c_double), ("ell", ctypes.c_double),
+                ("lam", ctypes.c_double), ("omega", ctypes.c_double), ("k0", ctypes.c_double),
+                ("dt", ctypes.c_double), ("tensor", ctypes.c_int32), ("integrator", ctypes.c_int32)]
+
+
+@dataclass
+class Params:
+    """Scalars of the model.  Defaults: BASELINE.json units a=eta=T=1."""
+    a: float = 1.0
+    eta: float = 1.0
+    ell: float = 10.0
+    lam: float = 2.0
+    omega: float = 2.0 * np.pi
+    k0: float = 1000.0
+    dt: float = 1e-3
+    tensor: int = RPY
+    integrator: int = HEUN
+
+    def c(self) -> _CParams:
+        return _CParams(self.a, self.eta, self.ell, self.lam, self.omega, self.k0, self.dt,
+                        int(self.tensor), int(self.integrator))
+
+
+_lib = None
+_dp = ctypes.POINTER(ctypes.c_double)
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = ctypes.CDLL(_build.build())
+        L.or_set_threads.argtypes = [ctypes.c_int]
+        L.or_get_threads.restype = ctypes.c_int
+        L.or_max_threads.restype = ctypes.c_int
+        L.or_forces.argtypes = [ctypes.c_int32, _dp, _dp, ctypes.c_double, ctypes.POINTER(_CParams), _dp]
+        L.or_dense_mobility.argtypes = [ctypes.c_int32, _dp, ctypes.c_double, ctypes.c_double, ctypes.c_int32, _dp]
+        L.or_mobility_apply.argtypes = [ctypes.c_int32, _dp, _dp, ctypes.c_double, ctypes.c_double,
+                                        ctypes.c_int32, _dp]
+        L.or_velocity.argtypes = [ctypes.c_int32, _dp, _dp, ctypes.c_double, ctypes.POINTER(_CParams), _dp, _dp]
+        L.or_step.argtypes = [ctypes.c_int32, _dp, _dp, ctypes.c_double, ctypes.c_int64, ctypes.c_int64,
+                              ctypes.POINTER(_CParams)]
+        L.or_step.restype = ctypes.c_int
+        L.or_step_record.argtypes = [ctypes.c_int32, _dp, _dp, ctypes.c_double, ctypes.c_int64, ctypes.c_int64,
+                                     ctypes.POINTER(_CParams), ctypes.c_int64, _dp]
+        L.or_step_record.restype = ctypes.c_int
+        _lib = L
+    return _lib
+
+
+def _d(x):
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    return x, x.ctypes.data_as(_dp)
+
+
+def set_threads(n: int) -> None:
+    lib().or_set_threads(int(n))
+
+
+def max_threads() -> int:
+    return int(lib().or_max_threads())
+
+
+def forces(X, phi, t, p: Params):
+    """Eq. (4).  X [N][3], phi [S] -> F [N][3]."""
+    X, Xp = _d(X)
+    phi, pp = _d(phi)
+    S = phi.shape[0]
+    assert X.shape == (2 * S, 3)
+    F = np.empty_like(X)
+    cp = p.c()
+    lib().or_forces(S, Xp, pp, float(t), ctypes.byref(cp), F.ctypes.data_as(_dp))
+    return F
+
+
+def dense_mobility(X, a, eta, tensor):
+    """Eq. (3a,b) entry by entry.  X [N][3] -> H [3N][3N]."""
+    X, Xp = _d(X)
+    N = X.shape[0]
+    H = np.empty((3 * N, 3 * N), dtype=np.float64)
+    lib().or_dense_mobility(N, Xp, float(a), float(eta), int(tensor), H.ctypes.data_as(_dp))
+    return H
+
+
+def mobility_apply(X, F, a, eta, tensor):
+    """u = H(X) F, matrix free.  X, F [N][3] -> u [N][3]."""
+    X, Xp = _d(X)
+    F, Fp = _d(F)
+    assert X.shape == F.shape and X.shape[1] == 3
+    u = np.empty_like(X)
+    lib().or_mobility_apply(X.shape[0], Xp, Fp, float(a), float(eta), int(tensor), u.ctypes.data_as(_dp))
+    return u
+
+
+def velocity(X, phi, t, p: Params):
+    X, Xp = _d(X)
+    phi, pp = _d(phi)
+    V = np.empty_like(X)
+    W = np.empty_like(X)
+    cp = p.c()
+    lib().or_velocity(phi.shape[0], Xp, pp, float(t), ctypes.byref(cp), V.ctypes.data_as(_dp),
+                      W.ctypes.data_as(_dp))
+    return V
+
+
+def step(X, phi, t0, n_done, n_steps, p: Params):
+    """n_steps explicit steps from step index n_done; returns the new X (input untouched)."""
+    X = np.array(X, dtype=np.float64, order="C", copy=True)
+    phi, pp = _d(phi)
+    assert X.shape == (2 * phi.shape[0], 3)
+    cp = p.c()
+    rc = lib().or_step(phi.shape[0], X.ctypes.data_as(_dp), pp, float(t0), int(n_done), int(n_steps),
+                       ctypes.byref(cp))
+    if rc:
+        raise MemoryError("or_step")
+    return X
+
+
+def step_record(X, phi, t0, n_done, n_steps, p: Params, stride: int):
+    """As step(), also returning the positions after every stride-th step: (X, traj[k][N][3])."""
+    X = np.array(X, dtype=np.float64, order="C", copy=True)
+    phi, pp = _d(phi)
+    cp = p.c()
+    traj = np.empty((n_steps // stride,) + X.shape, dtype=np.float64)
+    rc = lib().or_step_record(phi.shape[0], X.ctypes.data_as(_dp), pp, float(t0), int(n_done), int(n_steps),
+                              ctypes.byref(cp), int(stride), traj.ctypes.data_as(_dp))
+    if rc:
+        raise MemoryError("or_step_record")
+    return X, traj

@@ -1,0 +1,223 @@
+/*
+ * ds_oracle.c -- CPU ORACLE for the active-dumbbell hot path of arXiv 1004.1932
+ * (Putz, Dunkel, Yeomans, "CUDA simulations of active dumbbell suspensions").
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  It is a plain, slow, double-precision
+ * restatement of the paper's equations, written so that a reader can check every line
+ * against the paper by eye.  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may call it.  It shares no code, header, table or
+ * helper with the CUDA library under paper_1004_1932_b200/csrc, and neither includes the
+ * other.
+ *
+ * What it computes (citations are lines of /root/reference/PAPER.md):
+ *   or_forces            Eq. (4)   PAPER.md:63-67   spring + stroke force per dumbbell
+ *   or_dense_mobility    Eq. (3a,b) PAPER.md:57-59  the full 3N x 3N tensor, entry by entry,
+ *                                                   in the paper's own form (the "full
+ *                                                   tensor" method of PAPER.md:230)
+ *   or_mobility_apply    Eq. (1a) deterministic part, PAPER.md:38, 77:
+ *                        u_(alpha i) = sum_beta H_(alpha i)(beta j) F_(beta j), matrix free
+ *   or_velocity          forces followed by the mobility apply
+ *   or_step              explicit Euler / one-step Heun predictor-corrector
+ *
+ * Readings of the paper used here:
+ *   R2  Heun = explicit trapezoid: X* = X + dt V(X,t); X' = X + dt/2 (V(X,t) + V(X*,t+dt)).
+ *   R4  Eq. (3b) is applied for every r > 0; no overlap branch (the paper has none).
+ *   R5  the intra-dumbbell pair is an ordinary beta != alpha pair (Eq. A16b).
+ *   R6  first sphere of a dumbbell gets +g n, the second -g n, n pointing first -> second,
+ *       g = k0 (d - L(t)); this is F = -dU/dX for U of Eq. (4).
+ *   R7  t = t0 + n dt formed from the integer step count, never accumulated.
+ *   R9  one radius a for all spheres.
+ *
+ * Parity pins: every function here is pinned by tests/test_oracle_pins.py against closed
+ * forms, textbook series and invariants (P1-P10 of SURVEY.md 8(c)); nothing is "parity
+ * unpinned".
+ *
+ * Storage: 0-based; dumbbell s owns spheres 2s and 2s+1 (paper, 1-based: 2s-1 and 2s,
+ * PAPER.md:63).  X, F, u are [N][3] row-major doubles, N = 2S.
+ *
+ * Summation: ascending beta with Neumaier-compensated accumulation per component, so that
+ * the oracle is the more exact side of every comparison (R12).  Threads (OpenMP over
+ * alpha) do not change any result bit: each alpha is summed by one thread in fixed order.
+ */
+#include <math.h>
+#include <stddef.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define OR_OSEEN 0
+#define OR_RPY 1
+#define OR_EULER 0
+#define OR_HEUN 1
+
+static const double OR_PI = 3.14159265358979323846264338327950288;
+
+typedef struct {
+    double a;      /* sphere radius  */
+    double eta;    /* viscosity (paper: mu)  */
+    double ell;    /* mean dumbbell length  */
+    double lambda; /* stroke amplitude  */
+    double omega;  /* driving angular frequency 2 pi / T PAPER.md:67  */
+    double k0;     /* spring constant  */
+    double dt;     /* time step */
+    int32_t tensor;     /* OR_OSEEN: first line of (3b) only; OR_RPY: both */
+    int32_t integrator; /* OR_EULER or OR_HEUN                           */
+} or_params;
+
+static int g_threads = 1;
+
+void or_set_threads(int n) { g_threads = n < 1 ? 1 : n; }
+
+int or_get_threads(void) { return g_threads; }
+
+int or_max_threads(void) {
+#ifdef _OPENMP
+    return omp_get_num_procs();
+#else
+    return 1;
+#endif
+}
+
+/* Neumaier's compensated sum: s + c is the running total. */
+static inline void nsum(double *s, double *c, double x) {
+    double t = *s + x;
+    if (fabs(*s) >= fabs(x))
+        *c += (*s - t) + x;
+    else
+        *c += (x - t) + *s;
+    *s = t;
+}
+
+/* Eq. (4).  U^s = (k0/2) [d^s - L^s(t)]^2, L^s(t) = ell + lambda sin(omega t + phi^s),
+ * d^s = |X_{2s+1} - X_{2s}|, F = -dU/dX.  With n = (X_{2s+1}-X_{2s})/d:
+ *   F_{2s} = +k0 (d-L) n,  F_{2s+1} = -k0 (d-L) n.                                         */
+void or_forces(int32_t S, const double *X, const double *phi, double t, const or_params *p, double *F) {
+    for (int32_t s = 0; s < S; ++s) {
+        const double *x1 = X + 6 * (size_t)s, *x2 = x1 + 3;
+        double sv[3] = {x2[0] - x1[0], x2[1] - x1[1], x2[2] - x1[2]};
+        double d = sqrt(sv[0] * sv[0] + sv[1] * sv[1] + sv[2] * sv[2]);
+        double L = p->ell + p->lambda * sin(p->omega * t + phi[s]);
+        double g = p->k0 * (d - L);
+        for (int i = 0; i < 3; ++i) {
+            double n = sv[i] / d;
+            F[6 * (size_t)s + i] = g * n;
+            F[6 * (size_t)s + 3 + i] = -(g * n);
+        }
+    }
+}
+
+/* Eq. (3a), (3b), written entry by entry exactly as printed:
+ *   H_(a i)(a j) = delta_ij / (6 pi mu a)
+ *   H_(a i)(b j) = 1/(8 pi mu r) (delta_ij + r_i r_j / r^2)
+ *                + 2 a^2/(24 pi mu r^3) (delta_ij - 3 r_i r_j / r^2),   r = x_a - x_b.
+ * Oseen keeps the first line only.  H is [3N][3N] row-major, row 3a+i, column 3b+j. */
+void or_dense_mobility(int32_t N, const double *X, double a, double eta, int32_t tensor, double *H) {
+    size_t M = 3 * (size_t)N;
+    for (int32_t al = 0; al < N; ++al) {
+        for (int32_t be = 0; be < N; ++be) {
+            for (int i = 0; i < 3; ++i) {
+                for (int j = 0; j < 3; ++j) {
+                    double dij = (i == j) ? 1.0 : 0.0, h;
+                    if (al == be) {
+                        h = dij / (6.0 * OR_PI * eta * a);
+                    } else {
+                        double rv[3] = {X[3 * al] - X[3 * be], X[3 * al + 1] - X[3 * be + 1],
+                                        X[3 * al + 2] - X[3 * be + 2]};
+                        double r = sqrt(rv[0] * rv[0] + rv[1] * rv[1] + rv[2] * rv[2]);
+                        double rr = rv[i] * rv[j] / (r * r);
+                        h = 1.0 / (8.0 * OR_PI * eta * r) * (dij + rr);
+                        if (tensor == OR_RPY)
+                            h += 2.0 * a * a / (24.0 * OR_PI * eta * r * r * r) * (dij - 3.0 * rr);
+                    }
+                    H[(3 * (size_t)al + i) * M + 3 * (size_t)be + j] = h;
+                }
+            }
+        }
+    }
+}
+
+/* Deterministic part of Eq. (1a), PAPER.md:38 with T = 0, matrix free:
+ *   u_a = F_a/(6 pi mu a) + sum_{b != a} T(r_ab) F_b.
+ * With r = x_a - x_b, r2 = r.r, rF = r.F_b, Eq. (3b) contracted with F_b is
+ *   Oseen: (1/(8 pi mu)) (1/r) [ F_b + r (rF / r2) ]
+ *   RPY  : (1/(8 pi mu)) (1/r) [ (1 + 2a^2/(3 r2)) F_b + (1 - 2a^2/r2) (rF / r2) r ]
+ * (the second line of (3b), 2a^2/(24 pi mu r^3) (delta - 3 rr/r2), equals
+ *  (1/(8 pi mu r)) [ (2a^2/(3 r2)) delta - (2a^2/r2) rr/r2 ]).                           */
+void or_mobility_apply(int32_t N, const double *X, const double *F, double a, double eta, int32_t tensor,
+                       double *u) {
+    const double self = 1.0 / (6.0 * OR_PI * eta * a);
+    const double pre = 1.0 / (8.0 * OR_PI * eta);
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static) num_threads(g_threads) if (g_threads > 1)
+#endif
+    for (int32_t al = 0; al < N; ++al) {
+        double s[3] = {0, 0, 0}, c[3] = {0, 0, 0};
+        const double *xa = X + 3 * (size_t)al;
+        for (int32_t be = 0; be < N; ++be) {
+            if (be == al) continue;
+            const double *xb = X + 3 * (size_t)be, *fb = F + 3 * (size_t)be;
+            double r[3] = {xa[0] - xb[0], xa[1] - xb[1], xa[2] - xb[2]};
+            double r2 = r[0] * r[0] + r[1] * r[1] + r[2] * r[2];
+            double rinv = 1.0 / sqrt(r2);
+            double rF = r[0] * fb[0] + r[1] * fb[1] + r[2] * fb[2];
+            double cd = 1.0, cr = rF / r2;
+            if (tensor == OR_RPY) {
+                cd = 1.0 + 2.0 * a * a / (3.0 * r2);
+                cr = (1.0 - 2.0 * a * a / r2) * (rF / r2);
+            }
+            for (int i = 0; i < 3; ++i) nsum(&s[i], &c[i], (cd * fb[i] + cr * r[i]) * rinv);
+        }
+        for (int i = 0; i < 3; ++i) u[3 * (size_t)al + i] = self * F[3 * (size_t)al + i] + pre * (s[i] + c[i]);
+    }
+}
+
+/* V(X, t) = H(X) F(X, t): the right-hand side of Eq. (1a) in the deterministic limit. */
+void or_velocity(int32_t S, const double *X, const double *phi, double t, const or_params *p, double *V,
+                 double *Fwork) {
+    or_forces(S, X, phi, t, p, Fwork);
+    or_mobility_apply(2 * S, X, Fwork, p->a, p->eta, p->tensor, V);
+}
+
+/* n_steps explicit steps from step index n_done (reading R2).
+ * t_n = t0 + n dt (R7).  X is updated in place.  Returns 0, or -1 if out of memory.       */
+int or_step(int32_t S, double *X, const double *phi, double t0, int64_t n_done, int64_t n_steps,
+            const or_params *p) {
+    size_t M = 6 * (size_t)S;
+    double *buf = (double *)malloc(4 * M * sizeof(double));
+    if (!buf) return -1;
+    double *V1 = buf, *V2 = buf + M, *Xp = buf + 2 * M, *Fw = buf + 3 * M;
+    for (int64_t n = n_done; n < n_done + n_steps; ++n) {
+        double t = t0 + (double)n * p->dt;
+        or_velocity(S, X, phi, t, p, V1, Fw);
+        if (p->integrator == OR_EULER) {
+            for (size_t k = 0; k < M; ++k) X[k] = X[k] + p->dt * V1[k];
+        } else {
+            double t1 = t0 + (double)(n + 1) * p->dt;
+            for (size_t k = 0; k < M; ++k) Xp[k] = X[k] + p->dt * V1[k];
+            or_velocity(S, Xp, phi, t1, p, V2, Fw);
+            for (size_t k = 0; k < M; ++k) X[k] = X[k] + 0.5 * p->dt * (V1[k] + V2[k]);
+        }
+    }
+    free(buf);
+    return 0;
+}
+
+/* Same as or_step, but also records the positions after every `stride`-th step into
+ * traj[(k)][N][3], k = 0 .. n_steps/stride - 1 (used by the observable pins, Eq. 11).     */
+int or_step_record(int32_t S, double *X, const double *phi, double t0, int64_t n_done, int64_t n_steps,
+                   const or_params *p, int64_t stride, double *traj) {
+    size_t M = 6 * (size_t)S;
+    int64_t k = 0;
+    for (int64_t n = 0; n < n_steps; ++n) {
+        int rc = or_step(S, X, phi, t0, n_done + n, 1, p);
+        if (rc) return rc;
+        if ((n + 1) % stride == 0) {
+            memcpy(traj + (size_t)k * M, X, M * sizeof(double));
+            ++k;
+        }
+    }
+    return 0;
+}

@@ -1,0 +1,371 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (no GPU).
+
+Each test names the pin (P1-P10 of SURVEY.md 8(c), plus extras) and the passage it rests on.
+None of them re-types the oracle's formula: they use closed forms for special geometries,
+textbook series, identities of Stokes flow, invariants, numerical differentiation of the
+paper's potential, and brute force through the dense tensor.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from oracle import OSEEN, RPY, EULER, HEUN, Params
+from paper_1004_1932_b200 import inputs
+
+PI = np.pi
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def two_spheres(r, direction=(1.0, 0.0, 0.0)):
+    d = np.asarray(direction, float)
+    d = d / np.linalg.norm(d)
+    return np.stack([np.zeros(3), r * d])
+
+
+# ----------------------------------------------------------------------------- P1, P2
+@pytest.mark.parametrize("r", [2.5, 7.0, 123.0])
+def test_P1_oseen_point_force_closed_form(r):
+    """PAPER.md:57-61 / 306-309: a unit force on sphere 2 moves sphere 1 with 1/(4 pi eta r)
+    along the line of centres (kappa = (4 pi mu)^-1 in 1d, A6) and 1/(8 pi eta r) normal to it;
+    sphere 2 itself moves with 1/(6 pi eta a)."""
+    a, eta = 0.7, 1.3
+    X = two_spheres(r)
+    for comp, expect in [(0, 1 / (4 * PI * eta * r)), (1, 1 / (8 * PI * eta * r)), (2, 1 / (8 * PI * eta * r))]:
+        F = np.zeros((2, 3))
+        F[1, comp] = 1.0
+        u = oracle.mobility_apply(X, F, a, eta, OSEEN)
+        want = np.zeros((2, 3))
+        want[0, comp] = expect
+        want[1, comp] = 1 / (6 * PI * eta * a)
+        np.testing.assert_allclose(u, want, rtol=1e-14, atol=1e-18)
+
+
+def _series():
+    c = {}
+    for line in open(os.path.join(GOLD, "two_sphere_series.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        k, c1, c3 = line.split()
+        c[k] = (float(c1), float(c3))
+    return c
+
+
+@pytest.mark.parametrize("rho", [2.0, 3.5, 10.0, 50.0])
+def test_P2_two_sphere_sedimentation_series(rho):
+    """tests/golden/two_sphere_series.txt: equal forces on two equal spheres.  RPY gives
+    U/U0 = 1 + c1/rho + c3/rho^3 exactly, Oseen 1 + c1/rho (textbook reflections series)."""
+    a, eta = 1.0, 1.0
+    c = _series()
+    U0 = 1 / (6 * PI * eta * a)
+    X = two_spheres(rho * a, direction=(0.0, 0.0, 1.0))
+    for comp, key in [(2, "parallel"), (0, "perpendicular"), (1, "perpendicular")]:
+        F = np.zeros((2, 3))
+        F[:, comp] = 1.0
+        c1, c3 = c[key]
+        u = oracle.mobility_apply(X, F, a, eta, RPY)
+        np.testing.assert_allclose(u[:, comp] / U0, 1 + c1 / rho + c3 / rho ** 3, rtol=1e-14)
+        u = oracle.mobility_apply(X, F, a, eta, OSEEN)
+        np.testing.assert_allclose(u[:, comp] / U0, 1 + c1 / rho, rtol=1e-14)
+        other = [k for k in range(3) if k != comp]
+        assert np.abs(u[:, other]).max() < 1e-17
+
+
+def test_rpy_is_oseen_plus_a2_over_3_laplacian():
+    """Finite-size correction of two equal spheres = (a^2/6 + a^2/6) Laplacian of the Stokeslet
+    (Faxen; Rotne & Prager ref. [26]).  The Laplacian is taken numerically from the oracle's own
+    Oseen tensor, so the second line of Eq. (3b) (coefficient 2a^2/24, the -3, the r^-3) is pinned
+    by the first line, not by re-typing it."""
+    a, eta = 1.3, 0.9
+    r0 = np.array([3.1, -2.2, 4.5])
+    h = 1e-3
+
+    def block(r, tensor):
+        return oracle.dense_mobility(np.stack([r, np.zeros(3)]), a, eta, tensor)[0:3, 3:6]
+
+    lap = -6 * block(r0, OSEEN)
+    for k in range(3):
+        e = np.zeros(3)
+        e[k] = h
+        lap = lap + block(r0 + e, OSEEN) + block(r0 - e, OSEEN)
+    lap /= h * h
+    diff = block(r0, RPY) - block(r0, OSEEN)
+    np.testing.assert_allclose(diff, a * a / 3 * lap, rtol=2e-6, atol=1e-9 * np.abs(diff).max())
+
+
+def test_tensor_is_divergence_free():
+    """d/dx_(beta j) H_(alpha i)(beta j) = 0 (incompressibility), both tensors."""
+    a, eta, h = 1.0, 1.0, 1e-4
+    rng = np.random.default_rng(5)
+    X = np.stack([np.zeros(3), rng.uniform(3, 6, 3)])
+    for tensor in (OSEEN, RPY):
+        div = np.zeros(3)
+        for j in range(3):
+            Xp, Xm = X.copy(), X.copy()
+            Xp[1, j] += h
+            Xm[1, j] -= h
+            Hp = oracle.dense_mobility(Xp, a, eta, tensor)[0:3, 3:6]
+            Hm = oracle.dense_mobility(Xm, a, eta, tensor)[0:3, 3:6]
+            div += (Hp[:, j] - Hm[:, j]) / (2 * h)
+        scale = np.abs(oracle.dense_mobility(X, a, eta, tensor)[0:3, 3:6]).max() / np.linalg.norm(X[1])
+        assert np.abs(div).max() < 1e-6 * scale
+
+
+# ----------------------------------------------------------------------------- P3, P4, P6
+@pytest.mark.parametrize("tensor", [OSEEN, RPY])
+def test_P3_symmetry(tensor):
+    """Eq. (3) is symmetric in (alpha i)(beta j) (needed by Eq. (2)): G.MF = F.MG."""
+    X, F = inputs.apply_case(200, 11, 12)
+    G = np.random.default_rng(13).standard_normal(F.shape)
+    lhs = np.sum(G * oracle.mobility_apply(X, F, 1.0, 1.0, tensor))
+    rhs = np.sum(F * oracle.mobility_apply(X, G, 1.0, 1.0, tensor))
+    assert abs(lhs - rhs) <= 1e-13 * max(abs(lhs), abs(rhs), 1.0)
+    H = oracle.dense_mobility(X[:40], 1.0, 1.0, tensor)
+    assert np.array_equal(H, H.T) or np.abs(H - H.T).max() < 1e-17
+
+
+def test_P4_rpy_positive_definite_beyond_contact():
+    """H positive definite for r > 2a, so the Cholesky factor of Eq. (2) exists."""
+    w = inputs.config2()
+    H = oracle.dense_mobility(w.pos[0], 1.0, 1.0, RPY)
+    np.linalg.cholesky(H)
+    X = two_spheres(2.0 + 1e-9)
+    ev = np.linalg.eigvalsh(oracle.dense_mobility(X, 1.0, 1.0, RPY))
+    assert ev.min() > 0
+    F = np.random.default_rng(3).standard_normal((w.N, 3))
+    assert np.sum(F * oracle.mobility_apply(w.pos[0], F, 1.0, 1.0, RPY)) > 0
+    # the Oseen truncation is not: the relative mode of two spheres goes negative at r < 1.5 a
+    ev = np.linalg.eigvalsh(oracle.dense_mobility(two_spheres(1.4), 1.0, 1.0, OSEEN))
+    assert ev.min() < 0
+
+
+@pytest.mark.parametrize("tensor", [OSEEN, RPY])
+@pytest.mark.parametrize("N", [1, 2, 3, 17, 64])
+def test_P6_dense_tensor_brute_force(N, tensor):
+    """the paper's own 'full tensor' method, H built entry by entry in the printed
+    form of Eq. (3), times F, equals the matrix-free sum (which uses the contracted form)."""
+    X, F = inputs.ragged_case(N, 100 + N)
+    a, eta = 0.8, 1.7
+    u = oracle.mobility_apply(X, F, a, eta, tensor)
+    H = oracle.dense_mobility(X, a, eta, tensor)
+    np.testing.assert_allclose(u.ravel(), H @ F.ravel(), rtol=0, atol=2e-15 * np.abs(u).max())
+
+
+@pytest.mark.parametrize("tensor", [OSEEN, RPY])
+def test_translation_rotation_permutation(tensor):
+    """The tensor depends on x_alpha - x_beta only; it is an isotropic tensor function (rotating
+    positions and forces rotates velocities); relabelling spheres relabels velocities."""
+    X, F = inputs.ragged_case(33, 7)
+    u = oracle.mobility_apply(X, F, 1.0, 1.0, tensor)
+    s = np.abs(u).max()
+    u_t = oracle.mobility_apply(X + np.array([3.0, -40.0, 7.5]), F, 1.0, 1.0, tensor)
+    assert np.abs(u_t - u).max() < 1e-12 * s
+    Q, _ = np.linalg.qr(np.random.default_rng(1).standard_normal((3, 3)))
+    u_r = oracle.mobility_apply(X @ Q.T, F @ Q.T, 1.0, 1.0, tensor)
+    assert np.abs(u_r - u @ Q.T).max() < 1e-13 * s
+    perm = np.random.default_rng(2).permutation(33)
+    u_p = oracle.mobility_apply(X[perm], F[perm], 1.0, 1.0, tensor)
+    assert np.abs(u_p - u[perm]).max() < 1e-14 * s
+    # linear in F; scales as 1/eta
+    u2 = oracle.mobility_apply(X, 2.5 * F, 1.0, 2.0, tensor)
+    assert np.abs(u2 - 1.25 * u).max() < 1e-14 * s
+
+
+# ----------------------------------------------------------------------------- P5
+def test_P5_forces_are_minus_grad_U_force_free_torque_free():
+    """Eq. (4): F = -dU/dX with U = sum (k0/2)(d - L(t))^2, checked by central
+    differences of U; Eq. (A22)-(A24) PAPER.md:445-460: each dumbbell is force free (bitwise) and
+    torque free (F parallel to n)."""
+    w = inputs.config2()
+    p = Params(k0=37.0)
+    t = 0.3731
+    rng = np.random.default_rng(9)
+    X = w.pos[0] + rng.uniform(-0.7, 0.7, w.pos[0].shape)   # off the minima
+    phi = w.phase[0]
+
+    def U(Xq):
+        d = np.linalg.norm(Xq[1::2] - Xq[0::2], axis=1)
+        L = p.ell + p.lam * np.sin(p.omega * t + phi)
+        return 0.5 * p.k0 * np.sum((d - L) ** 2)
+
+    F = oracle.forces(X, phi, t, p)
+    h = 1e-6
+    for (al, i) in [(0, 0), (1, 2), (50, 1), (127, 0), (64, 2)]:
+        Xp, Xm = X.copy(), X.copy()
+        Xp[al, i] += h
+        Xm[al, i] -= h
+        assert abs(F[al, i] + (U(Xp) - U(Xm)) / (2 * h)) < 1e-6 * np.abs(F).max()
+    assert np.array_equal(F[0::2], -F[1::2])
+    n = X[1::2] - X[0::2]
+    assert np.abs(np.cross(n, F[0::2])).max() < 1e-12 * np.abs(F).max() * np.abs(n).max()
+    # sign (reading R6): a stretched spring (d > L) pulls sphere 1 towards sphere 2
+    Xs = np.array([[0.0, 0, 0], [15.0, 0, 0]])
+    Fs = oracle.forces(Xs, np.array([0.0]), 0.0, Params())
+    assert Fs[0, 0] > 0 and Fs[1, 0] < 0 and abs(Fs[0, 0] - 1000.0 * 5.0) < 1e-9
+    # at the potential minima (input recipe) the force vanishes at t = 0
+    F0 = oracle.forces(w.pos[0], phi, 0.0, Params())
+    assert np.abs(F0).max() < 1e-9
+
+
+# ----------------------------------------------------------------------------- P7, P8
+def test_P7_isolated_dumbbell_does_not_translate():
+    """I^sigma = 0, Eq. (A44); scallop theorem PAPER.md:22; the authors' acceptance
+    check 'single dumbbells did not translate'."""
+    n = np.array([1.0, 2.0, -0.5])
+    n /= np.linalg.norm(n)
+    phi = np.array([0.9])
+    R0 = np.array([[3.0, -1.0, 2.0]])
+    X0 = inputs.place_spheres(R0, n[None], phi)
+    for tensor in (OSEEN, RPY):
+        p = Params(tensor=tensor)
+        V = oracle.velocity(X0 + np.array([[0.3, 0, 0], [0, 0, 0]]), phi, 0.1, p)
+        assert np.abs(V[0] + V[1]).max() <= 1e-15 * np.abs(V).max()
+        X = oracle.step(X0, phi, 0.0, 0, 3000, p)
+        assert np.abs(0.5 * (X[0] + X[1]) - R0[0]).max() < 1e-12
+        nn = (X[1] - X[0]) / np.linalg.norm(X[1] - X[0])
+        assert np.abs(nn - n).max() < 1e-12          # and does not rotate
+        assert abs(np.linalg.norm(X[1] - X[0]) - 10.0) < 2.5   # still a dumbbell of length ~ ell
+
+
+def test_P8_isolated_dumbbell_length_relaxation_A37():
+    """Eq. (A29a), (A36), (A37) PAPER.md:484-535 with the Oseen tensor: for one dumbbell
+    d(d)/dt = b f1, b = (4 kappa / d)(1 - 2d/(3a)), kappa = 1/(8 pi mu), f1 = force on sphere 1
+    along n.  Pins self mobility, the factor 2 of the parallel Oseen mode and the force sign."""
+    a, eta, k0 = 1.0, 1.0, 1000.0
+    p = Params(a=a, eta=eta, k0=k0, tensor=OSEEN)
+    phi = np.array([0.4])
+    t = 0.17
+    for d in (8.3, 10.0, 11.9):
+        X = np.array([[0.0, 0, 0], [0.0, d, 0]])
+        V = oracle.velocity(X, phi, t, p)
+        ddot = V[1, 1] - V[0, 1]
+        L = p.ell + p.lam * np.sin(p.omega * t + phi[0])
+        f1 = k0 * (d - L)                         # on sphere 1, along n = +y (R6)
+        kappa = 1 / (8 * PI * eta)
+        b = 4 * kappa / d * (1 - 2 * d / (3 * a))
+        assert abs(ddot - b * f1) <= 1e-13 * abs(b * f1)
+
+
+def test_P8_lag_amplitude_and_stroke_frequency():
+    """Linear response of d - L to L(t) = ell + lam sin(omega t + phi) with relaxation
+    rate Gamma = -k0 b(ell) from (A37): amplitude lam omega / sqrt(Gamma^2 + omega^2); the lag is
+    the 'sphere positions lag very slightly behind the potentials' of PAPER.md:238.  Pins the
+    time dependence of the rest length and the integrator's time argument."""
+    lam = 0.05
+    p = Params(lam=lam, tensor=OSEEN, dt=5e-4)
+    phi = np.array([1.1])
+    X0 = inputs.place_spheres(np.zeros((1, 3)), np.array([[0.0, 0, 1.0]]), phi, lam=lam)
+    nsteps = 6000
+    _, traj = oracle.step_record(X0, phi, 0.0, 0, nsteps, p, 1)
+    tt = p.dt * np.arange(1, nsteps + 1)
+    d = np.linalg.norm(traj[:, 1] - traj[:, 0], axis=1)
+    dev = (d - (p.ell + lam * np.sin(p.omega * tt + phi[0])))[-2000:]     # last period
+    kappa = 1 / (8 * PI * p.eta)
+    Gamma = -p.k0 * 4 * kappa / p.ell * (1 - 2 * p.ell / (3 * p.a))
+    want = lam * p.omega / np.hypot(Gamma, p.omega)
+    got = 0.5 * (dev.max() - dev.min())
+    assert abs(got - want) < 0.01 * want
+    # d itself oscillates with the stroke period T = 1 about ell with amplitude ~ lam
+    dl = d[-2000:]
+    assert abs(0.5 * (dl.max() - dl.min()) - lam * Gamma / np.hypot(Gamma, p.omega)) < 0.01 * lam
+    assert abs(dl.mean() - p.ell) < 1e-3 * lam
+
+
+# ----------------------------------------------------------------------------- P9
+def _pair_drift(a, ell, lam, D, dphi, tensor=RPY, k0=None, steps_per_period=1000):
+    """Displacement of both centres over the second stroke period (first discarded,
+    PAPER.md:238) for two dumbbells aligned on the x axis, centres D apart."""
+    if k0 is None:
+        # same integrator loading Gamma dt ~ 0.09 as the paper's Fig. 1 (reading R1)
+        k0 = 90.2 / (2 * (1 / (6 * PI * a) - 1 / (4 * PI * ell)))
+    p = Params(a=a, ell=ell, lam=lam, k0=k0, dt=1.0 / steps_per_period, tensor=tensor)
+    phi = np.array([0.3, 0.3 + dphi])
+    R = np.array([[0.0, 0, 0], [D, 0, 0]])
+    n = np.array([[1.0, 0, 0], [1.0, 0, 0]])
+    X0 = inputs.place_spheres(R, n, phi, ell=ell, lam=lam)
+    X1 = oracle.step(X0, phi, 0.0, 0, steps_per_period, p)
+    X2 = oracle.step(X1, phi, 0.0, steps_per_period, steps_per_period, p)
+    c1 = 0.5 * (X1[0::2] + X1[1::2])
+    c2 = 0.5 * (X2[0::2] + X2[1::2])
+    return (c2 - c1)[:, 0], np.abs((c2 - c1)[:, 1:]).max()
+
+
+def _eq10(a, ell, lam, D, dphi, omega=2 * PI, T=1.0):
+    """Eq. (10) PAPER.md:147 for S = 2 over one period: both centres move by
+    (9/16) a omega sin(phi2 - phi1) (lam/ell)^2 (ell/D)^4 T along +x."""
+    return 9.0 / 16.0 * a * omega * np.sin(dphi) * (lam / ell) ** 2 * (ell / D) ** 4 * T
+
+
+def test_P9_aligned_pair_vs_stroke_averaged_eq10():
+    """PAPER.md:147 Eq. (10), 160-162, Fig. 1: symmetric aligned dumbbells move in the same
+    direction with identical speeds, direction set by phi2 - phi1, no motion for phase differences
+    that are multiples of pi, displacement per stroke ~ D^-4, and the ratio to Eq. (10) tends to 1
+    as a/ell -> 0 at constant lam (Fig. 1c)."""
+    a, lam = 1.0, 1.0
+    dx, off = _pair_drift(a, 10.0, lam, 100.0, PI / 2)
+    assert off < 1e-15
+    assert dx[0] > 0 and dx[1] > 0 and abs(dx[0] - dx[1]) < 2e-3 * abs(dx[0])
+    ref = _eq10(a, 10.0, lam, 100.0, PI / 2)
+    assert 1.0 < dx.mean() / ref < 1.3            # a/ell = 0.1: above Eq. (10), Fig. 1(c)
+    dxm, _ = _pair_drift(a, 10.0, lam, 100.0, -PI / 2)
+    assert abs(dxm.mean() + dx.mean()) < 0.02 * dx.mean()      # reversed phase lag reverses the motion
+    for dphi in (0.0, PI):
+        d0, _ = _pair_drift(a, 10.0, lam, 100.0, dphi)
+        assert np.abs(d0).max() < 1e-3 * dx.mean()
+    dhalf, _ = _pair_drift(a, 10.0, lam, 100.0, PI / 6)        # sin(pi/6) = 1/2
+    assert abs(dhalf.mean() / dx.mean() - 0.5) < 0.02
+    dnear, _ = _pair_drift(a, 10.0, lam, 50.0, PI / 2)
+    assert abs(dnear.mean() / dx.mean() - 16.0) < 1.0          # D^-4
+    ratios = []
+    for ell in (5.0, 10.0, 20.0, 40.0):                        # a/ell = 0.2 ... 0.025, D = 10 ell
+        d, _ = _pair_drift(a, ell, lam, 10 * ell, PI / 2)
+        ratios.append(d.mean() / _eq10(a, ell, lam, 10 * ell, PI / 2))
+    assert all(r1 > r2 for r1, r2 in zip(ratios, ratios[1:])), ratios
+    assert 1.2 < ratios[0] < 1.5 and abs(ratios[-1] - 1.0) < 0.07, ratios
+    # Oseen and RPY agree to a few per cent in the dilute, slender regime
+    do, _ = _pair_drift(a, 10.0, lam, 100.0, PI / 2, tensor=OSEEN)
+    assert abs(do.mean() / dx.mean() - 1.0) < 0.05
+
+
+# ----------------------------------------------------------------------------- P10
+def test_P10_integrator_order():
+    """one-step Heun predictor-corrector is 2nd order, Euler 1st."""
+    X0, phase = inputs.random_suspension(3, 77, side=40.0)
+    T_end = 0.064
+    errs = {}
+    for integ in (EULER, HEUN):
+        pref = Params(integrator=HEUN, dt=T_end / 4096, k0=200.0)
+        Xref = oracle.step(X0, phase, 0.0, 0, 4096, pref)
+        e = []
+        for n in (64, 128, 256):
+            p = Params(integrator=integ, dt=T_end / n, k0=200.0)
+            e.append(np.abs(oracle.step(X0, phase, 0.0, 0, n, p) - Xref).max())
+        errs[integ] = e
+    rh = [errs[HEUN][i] / errs[HEUN][i + 1] for i in range(2)]
+    re = [errs[EULER][i] / errs[EULER][i + 1] for i in range(2)]
+    assert all(3.5 < r < 4.6 for r in rh), rh
+    assert all(1.8 < r < 2.3 for r in re), re
+
+
+def test_step_bookkeeping_time_from_step_index():
+    """Reading R7: t_n = t0 + n dt from the integer step count, so n steps in one call equal the
+    same n steps split over several calls, bit for bit; t0 shifts the stroke phase."""
+    w = inputs.config1()
+    p = Params()
+    Xa = oracle.step(w.pos[0], w.phase[0], 0.25, 0, 40, p)
+    Xb = oracle.step(w.pos[0], w.phase[0], 0.25, 0, 15, p)
+    Xb = oracle.step(Xb, w.phase[0], 0.25, 15, 25, p)
+    assert np.array_equal(Xa, Xb)
+    # omega t0 = 2 pi * 1.0 is a full period: same forces as t0 = 0 up to rounding of the argument
+    F0 = oracle.forces(w.pos[0] * 1.01, w.phase[0], 0.0, p)
+    F1 = oracle.forces(w.pos[0] * 1.01, w.phase[0], 1.0, p)
+    assert np.abs(F0 - F1).max() < 1e-9 * np.abs(F0).max()
+    # threads do not change a bit
+    X, F = inputs.apply_case(300, 5, 6)
+    oracle.set_threads(1)
+    u1 = oracle.mobility_apply(X, F, 1.0, 1.0, RPY)
+    oracle.set_threads(4)
+    u4 = oracle.mobility_apply(X, F, 1.0, 1.0, RPY)
+    oracle.set_threads(1)
+    assert np.array_equal(u1, u4)
