@@ -1,0 +1,163 @@
+"""Thin ctypes binding of the C ABI in include/ds.h (argument marshalling only).
+
+Every step of the path runs in the CUDA kernels of csrc/; this module holds no arithmetic of
+the method and has NO CPU fallback: if libds.so cannot be built/loaded, or there is no sm_100
+device, the calls raise.  torch is used only for device memory and streams: any object with a
+`data_ptr()` (torch tensor, device or pinned/pageable host) or a numpy array is accepted as a
+buffer; the library itself tells host from device pointers.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+from . import build as _build
+
+F32, F64 = 0, 1
+OSEEN, RPY = 0, 1
+EULER, HEUN = 0, 1
+
+OK = 0
+ERR_INVALID_PARAM, ERR_NULL, ERR_CUDA, ERR_STATE, ERR_NO_DEVICE, ERR_ALLOC = -1, -2, -3, -4, -5, -6
+
+# every symbol include/ds.h declares (tests check that the built library exports all of them)
+SYMBOLS = ["ds_create", "ds_destroy", "ds_set_stream", "ds_set_state", "ds_get_state", "ds_forces",
+           "ds_mobility_apply", "ds_step", "ds_batch_step", "ds_velocity", "ds_set_tuning", "ds_launch_count",
+           "ds_strerror", "ds_last_cuda_error", "ds_version"]
+
+
+class DsError(RuntimeError):
+    def __init__(self, code, where):
+        self.code = code
+        L = lib()
+        msg = L.ds_strerror(code).decode()
+        cu = L.ds_last_cuda_error().decode()
+        super().__init__(f"{where}: {msg} ({code})" + (f" [{cu}]" if code == ERR_CUDA and cu else ""))
+
+
+class Params(ctypes.Structure):
+    """Mirror of ds_params (include/ds.h)."""
+    _fields_ = [("n_dumbbells", ctypes.c_int32), ("n_batch", ctypes.c_int32), ("precision", ctypes.c_int32),
+                ("tensor", ctypes.c_int32), ("integrator", ctypes.c_int32), ("device", ctypes.c_int32),
+                ("a", ctypes.c_double), ("eta", ctypes.c_double), ("ell", ctypes.c_double),
+                ("lam", ctypes.c_double), ("omega", ctypes.c_double), ("k0", ctypes.c_double),
+                ("dt", ctypes.c_double), ("stream", ctypes.c_void_p)]
+
+
+_lib = None
+
+
+def lib():
+    """Build (if stale) and load libds.so.  Raises if that fails: there is no fallback."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = ctypes.CDLL(path)
+        vp, i32, i64, dbl = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_double
+        L.ds_create.argtypes = [ctypes.POINTER(Params), ctypes.POINTER(vp)]
+        L.ds_destroy.argtypes = [vp]
+        L.ds_set_stream.argtypes = [vp, vp]
+        L.ds_set_state.argtypes = [vp, vp, vp, dbl]
+        L.ds_get_state.argtypes = [vp, vp, ctypes.POINTER(dbl)]
+        L.ds_forces.argtypes = [vp, vp]
+        L.ds_mobility_apply.argtypes = [vp, vp, vp, vp, i32]
+        L.ds_step.argtypes = [vp, i64]
+        L.ds_batch_step.argtypes = [vp, i64]
+        L.ds_velocity.argtypes = [vp, vp]
+        L.ds_set_tuning.argtypes = [vp, i32]
+        L.ds_launch_count.argtypes = [vp]
+        L.ds_launch_count.restype = i64
+        for f in ("ds_strerror", "ds_last_cuda_error", "ds_version"):
+            getattr(L, f).restype = ctypes.c_char_p
+        L.ds_strerror.argtypes = [ctypes.c_int]
+        _lib = L
+    return _lib
+
+
+def version():
+    return lib().ds_version().decode()
+
+
+def _ptr(x):
+    """Raw address of a torch tensor / numpy array (must be contiguous); None -> NULL."""
+    if x is None:
+        return None
+    if hasattr(x, "data_ptr"):
+        if not x.is_contiguous():
+            raise ValueError("buffer must be contiguous")
+        return ctypes.c_void_p(x.data_ptr())
+    if isinstance(x, np.ndarray):
+        if not x.flags["C_CONTIGUOUS"]:
+            raise ValueError("buffer must be contiguous")
+        return ctypes.c_void_p(x.ctypes.data)
+    if isinstance(x, int):
+        return ctypes.c_void_p(x)
+    raise TypeError(f"unsupported buffer type {type(x)}")
+
+
+def _check(code, where):
+    if code != OK:
+        raise DsError(code, where)
+
+
+class System:
+    """Owner of one ds_system handle; method names and arguments follow include/ds.h."""
+
+    def __init__(self, n_dumbbells, n_batch=1, precision=F64, tensor=RPY, integrator=HEUN, a=1.0, eta=1.0,
+                 ell=10.0, lam=2.0, omega=2.0 * np.pi, k0=1000.0, dt=1e-3, device=0, stream=None):
+        self._h = ctypes.c_void_p()
+        self.params = Params(int(n_dumbbells), int(n_batch), int(precision), int(tensor), int(integrator),
+                             int(device), float(a), float(eta), float(ell), float(lam), float(omega),
+                             float(k0), float(dt), ctypes.c_void_p(stream) if stream else None)
+        _check(lib().ds_create(ctypes.byref(self.params), ctypes.byref(self._h)), "ds_create")
+        self.S, self.N, self.B = int(n_dumbbells), 2 * int(n_dumbbells), int(n_batch)
+        self.precision = int(precision)
+
+    def destroy(self):
+        if self._h:
+            lib().ds_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()
+
+    def set_stream(self, stream):
+        _check(lib().ds_set_stream(self._h, ctypes.c_void_p(stream) if stream else None), "ds_set_stream")
+
+    def set_state(self, pos, phase, t0=0.0):
+        _check(lib().ds_set_state(self._h, _ptr(pos), _ptr(phase), float(t0)), "ds_set_state")
+
+    def get_state(self, pos=None):
+        t = ctypes.c_double()
+        _check(lib().ds_get_state(self._h, _ptr(pos), ctypes.byref(t)), "ds_get_state")
+        return t.value
+
+    def forces(self, F):
+        _check(lib().ds_forces(self._h, _ptr(F)), "ds_forces")
+
+    def velocity(self, V):
+        _check(lib().ds_velocity(self._h, _ptr(V)), "ds_velocity")
+
+    def mobility_apply(self, pos, F, u, n):
+        _check(lib().ds_mobility_apply(self._h, _ptr(pos), _ptr(F), _ptr(u), int(n)), "ds_mobility_apply")
+
+    def step(self, n_steps):
+        _check(lib().ds_step(self._h, int(n_steps)), "ds_step")
+
+    def batch_step(self, n_steps):
+        _check(lib().ds_batch_step(self._h, int(n_steps)), "ds_batch_step")
+
+    def set_tuning(self, j_splits=0):
+        _check(lib().ds_set_tuning(self._h, int(j_splits)), "ds_set_tuning")
+
+    def launch_count(self):
+        return int(lib().ds_launch_count(self._h))

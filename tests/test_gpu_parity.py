@@ -1,0 +1,273 @@
+"""Parity of the CUDA path (through the C ABI, include/ds.h) with the CPU oracle, element by element
+on the same seeded inputs.  Run on the B200 box: pytest -m gpu.
+
+Tolerances (BASELINE.json north_star; error norms SURVEY.md 8(c) R13):
+  mobility apply  FP64: ||u - u_or||_2 / ||u_or||_2 <= 1e-12     FP32: <= 1e-5
+  trajectory      FP32: max |X - X_or| <= 1e-4 ell after 1000 steps
+FP32 runs feed the oracle the SAME float32-rounded inputs (widened to double).
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_1004_1932_b200 import ds, inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL = {ds.F32: 1e-5, ds.F64: 1e-12}
+NPDT = {ds.F32: np.float32, ds.F64: np.float64}
+TDT = {ds.F32: torch.float32, ds.F64: torch.float64}
+ELL = inputs.ELL
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _device():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device (no CPU fallback exists)"
+    assert torch.cuda.get_device_capability(0)[0] == 10, "sm_100 device required"
+    oracle.set_threads(oracle.max_threads())   # bit-identical at any thread count
+    yield
+    oracle.set_threads(1)
+
+
+def rel_l2(u, ref):
+    return float(np.linalg.norm((u - ref).ravel()) / np.linalg.norm(ref.ravel()))
+
+
+def dev(x, precision):
+    return torch.as_tensor(np.ascontiguousarray(x, dtype=NPDT[precision]), device="cuda")
+
+
+def gpu_apply(X, F, precision, tensor, a=1.0, eta=1.0, j_splits=0, host=False):
+    n = X.shape[0]
+    with ds.System(1, precision=precision, tensor=tensor, a=a, eta=eta) as s:
+        if j_splits:
+            s.set_tuning(j_splits)
+        if host:
+            Xh = np.ascontiguousarray(X, dtype=NPDT[precision])
+            Fh = np.ascontiguousarray(F, dtype=NPDT[precision])
+            uh = np.full((n, 3), np.nan, dtype=NPDT[precision])
+            s.mobility_apply(Xh, Fh, uh, n)
+            return uh.astype(np.float64)
+        Xd, Fd = dev(X, precision), dev(F, precision)
+        ud = torch.full((n, 3), float("nan"), dtype=TDT[precision], device="cuda")
+        s.mobility_apply(Xd, Fd, ud, n)
+        torch.cuda.synchronize()
+        return ud.cpu().numpy().astype(np.float64)
+
+
+def oracle_apply(X, F, precision, tensor, a=1.0, eta=1.0):
+    Xr = np.asarray(X, dtype=NPDT[precision]).astype(np.float64)
+    Fr = np.asarray(F, dtype=NPDT[precision]).astype(np.float64)
+    return oracle.mobility_apply(Xr, Fr, a, eta, tensor)
+
+
+# --------------------------------------------------------------------------------- mobility apply
+@pytest.mark.parametrize("precision", [ds.F32, ds.F64])
+@pytest.mark.parametrize("tensor", [ds.OSEEN, ds.RPY])
+@pytest.mark.parametrize("N", [1, 2, 3, 17, 64, 255, 256, 257, 1000, 1027, 2048])
+def test_apply_parity_sizes(N, tensor, precision):
+    """Sizes below one tile, exactly one tile, ragged tails, several tiles and splits."""
+    X, F = inputs.ragged_case(N, 500 + N)
+    u = gpu_apply(X, F, precision, tensor, a=0.9, eta=1.3)
+    ref = oracle_apply(X, F, precision, tensor, a=0.9, eta=1.3)
+    assert np.isfinite(u).all()
+    assert rel_l2(u, ref) <= TOL[precision]
+
+
+@pytest.mark.parametrize("precision", [ds.F32, ds.F64])
+@pytest.mark.parametrize("tensor", [ds.OSEEN, ds.RPY])
+def test_apply_parity_config4_full_size(tensor, precision):
+    """BASELINE.json config 4: N = 4096 random suspension, forces N(0,1): the headline apply, in the
+    launch configuration bench.py times (library heuristic)."""
+    X, F = inputs.apply_case(4096, 1004, 2004)
+    u = gpu_apply(X, F, precision, tensor)
+    ref = oracle_apply(X, F, precision, tensor)
+    assert rel_l2(u, ref) <= TOL[precision]
+    # per-sphere check too: no single row is off by more than a few tolerances of the typical |u|
+    scale = np.sqrt(np.mean(ref ** 2))
+    assert np.abs(u - ref).max() <= 20 * TOL[precision] * scale
+
+
+@pytest.mark.parametrize("precision", [ds.F32, ds.F64])
+@pytest.mark.parametrize("j_splits", [1, 2, 5, 16])
+def test_apply_parity_forced_splits(j_splits, precision):
+    """The split-j partial-sum path and the single-block path give the same answer."""
+    X, F = inputs.apply_case(1536, 21, 22)
+    u = gpu_apply(X, F, precision, ds.RPY, j_splits=j_splits)
+    assert rel_l2(u, oracle_apply(X, F, precision, ds.RPY)) <= TOL[precision]
+
+
+@pytest.mark.parametrize("precision", [ds.F32, ds.F64])
+def test_apply_host_pointers_and_determinism(precision):
+    X, F = inputs.apply_case(700, 31, 32)
+    u_host = gpu_apply(X, F, precision, ds.RPY, host=True)
+    u_dev = gpu_apply(X, F, precision, ds.RPY)
+    u_dev2 = gpu_apply(X, F, precision, ds.RPY)
+    assert np.array_equal(u_host, u_dev)          # same kernels either way
+    assert np.array_equal(u_dev, u_dev2)          # fixed summation order: bitwise reproducible
+    assert rel_l2(u_dev, oracle_apply(X, F, precision, ds.RPY)) <= TOL[precision]
+
+
+@pytest.mark.parametrize("tensor", [ds.OSEEN, ds.RPY])
+def test_apply_scaling_sweep_16384(tensor):
+    """BASELINE.json config 5 sweep member N = 16384 (FP32), full parity."""
+    X, F = inputs.sweep_case(14)
+    u = gpu_apply(X, F, ds.F32, tensor)
+    assert rel_l2(u, oracle_apply(X, F, ds.F32, tensor)) <= TOL[ds.F32]
+
+
+def test_apply_two_sphere_closed_form_on_gpu():
+    """the GPU path itself reproduces the two-sphere Oseen closed form."""
+    r, a, eta = 7.0, 0.7, 1.3
+    X = np.array([[0.0, 0, 0], [r, 0, 0]])
+    F = np.array([[0.0, 0, 0], [1.0, 0, 0]])
+    u = gpu_apply(X, F, ds.F64, ds.OSEEN, a=a, eta=eta)
+    np.testing.assert_allclose(u[0, 0], 1 / (4 * np.pi * eta * r), rtol=1e-14)
+    np.testing.assert_allclose(u[1, 0], 1 / (6 * np.pi * eta * a), rtol=1e-14)
+
+
+# --------------------------------------------------------------------------------- forces / velocity
+def make_system(w, precision, tensor=ds.RPY, integrator=ds.HEUN, **kw):
+    sc = dict(w.scalars)
+    sc.update(kw)
+    s = ds.System(w.S, n_batch=w.B, precision=precision, tensor=tensor, integrator=integrator, a=sc["a"],
+                  eta=sc["eta"], ell=sc["ell"], lam=sc["lam"], omega=sc["omega"], k0=sc["k0"], dt=sc["dt"])
+    return s, oracle.Params(a=sc["a"], eta=sc["eta"], ell=sc["ell"], lam=sc["lam"], omega=sc["omega"], k0=sc["k0"],
+                            dt=sc["dt"], tensor=tensor, integrator=integrator)
+
+
+def rounded(w, precision):
+    return np.asarray(w.pos, dtype=NPDT[precision]).astype(np.float64)
+
+
+@pytest.mark.parametrize("precision", [ds.F32, ds.F64])
+def test_forces_and_velocity_parity(precision):
+    w = inputs.config2()
+    X0 = rounded(w, precision)
+    X0 = X0 + np.random.default_rng(4).uniform(-0.3, 0.3, X0.shape).astype(NPDT[precision]).astype(np.float64)
+    X0 = X0.astype(NPDT[precision]).astype(np.float64)
+    s, p = make_system(w, precision)
+    with s:
+        s.set_state(dev(X0, precision), torch.as_tensor(w.phase, device="cuda"), t0=0.37)
+        F = torch.empty((w.B, w.N, 3), dtype=TDT[precision], device="cuda")
+        V = torch.empty_like(F)
+        s.forces(F)
+        s.velocity(V)
+        torch.cuda.synchronize()
+        Fo = oracle.forces(X0[0], w.phase[0], 0.37, p)
+        Vo = oracle.velocity(X0[0], w.phase[0], 0.37, p)
+        assert rel_l2(F.cpu().numpy()[0].astype(np.float64), Fo) <= (1e-14 if precision == ds.F64 else 1e-7)
+        assert rel_l2(V.cpu().numpy()[0].astype(np.float64), Vo) <= TOL[precision]
+        Xb = torch.empty((w.B, w.N, 3), dtype=TDT[precision], device="cuda")
+        assert s.get_state(Xb) == pytest.approx(0.37)
+        assert np.array_equal(Xb.cpu().numpy().astype(np.float64), X0)
+
+
+# --------------------------------------------------------------------------------- stepping
+def gpu_steps(w, precision, n_steps, tensor=ds.RPY, integrator=ds.HEUN, t0=0.0, chunks=None, **kw):
+    s, p = make_system(w, precision, tensor, integrator, **kw)
+    with s:
+        X0 = rounded(w, precision)
+        s.set_state(dev(X0, precision), torch.as_tensor(w.phase, device="cuda"), t0=t0)
+        for c in (chunks or [n_steps]):
+            s.batch_step(c) if w.B > 1 else s.step(c)
+        out = torch.empty((w.B, w.N, 3), dtype=TDT[precision], device="cuda")
+        t = s.get_state(out)
+        torch.cuda.synchronize()
+        assert t == pytest.approx(t0 + n_steps * p.dt, rel=1e-12)
+        return out.cpu().numpy().astype(np.float64), X0, p
+
+
+def test_step_config1_fp64_full_run():
+    """C1: 1d line, S = 8, FP64, all 10^4 steps (10 stroke periods)."""
+    w = inputs.config1()
+    Xg, X0, p = gpu_steps(w, ds.F64, w.n_steps)
+    Xo = oracle.step(X0[0], w.phase[0], 0.0, 0, w.n_steps, p)
+    assert np.abs(Xg[0] - Xo).max() <= 1e-9 * ELL
+    assert np.abs(Xg[0, :, 1:]).max() == 0.0           # stays on the x axis exactly
+
+
+@pytest.mark.parametrize("precision,n_steps,tol", [(ds.F64, 10_000, 1e-8), (ds.F32, 1000, 1e-4), (ds.F32, 10_000, 1e-4)])
+def test_step_config2(precision, n_steps, tol):
+    """C2: 4x4x4 lattice; FP32 within 1e-4 ell after 1000 steps (north_star), FP64 over the full 10^4."""
+    w = inputs.config2()
+    Xg, X0, p = gpu_steps(w, precision, n_steps)
+    Xo = oracle.step(X0[0], w.phase[0], 0.0, 0, n_steps, p)
+    assert np.abs(Xg[0] - Xo).max() <= tol * ELL
+
+
+def test_step_config3_fp32_1000_steps():
+    """C3: S = 512 random suspension, FP32, first 1000 steps."""
+    w = inputs.config3()
+    Xg, X0, p = gpu_steps(w, ds.F32, 1000)
+    Xo = oracle.step(X0[0], w.phase[0], 0.0, 0, 1000, p)
+    assert np.abs(Xg[0] - Xo).max() <= 1e-4 * ELL
+
+
+@pytest.mark.parametrize("precision,tol", [(ds.F32, 1e-4), (ds.F64, 1e-10)])
+def test_step_config4_200_steps(precision, tol):
+    """C4: S = 2048 (N = 4096), the split-j + fused-epilogue path at full size."""
+    w = inputs.config4()
+    Xg, X0, p = gpu_steps(w, precision, 200)
+    Xo = oracle.step(X0[0], w.phase[0], 0.0, 0, 200, p)
+    assert np.abs(Xg[0] - Xo).max() <= tol * ELL
+
+
+def test_batch_step_config5_three_systems():
+    """C5: B = 64 systems of S = 256, FP32; parity on 3 of the 64 over 1000 steps."""
+    w = inputs.config5()
+    Xg, X0, p = gpu_steps(w, ds.F32, 1000)
+    for b in (0, 31, 63):
+        Xo = oracle.step(X0[b], w.phase[b], 0.0, 0, 1000, p)
+        assert np.abs(Xg[b] - Xo).max() <= 1e-4 * ELL
+
+
+@pytest.mark.parametrize("integrator", [ds.EULER, ds.HEUN])
+@pytest.mark.parametrize("tensor", [ds.OSEEN, ds.RPY])
+def test_step_integrators_tensors_chunking_t0(integrator, tensor):
+    """Euler and Heun, both tensors, t0 != 0, odd step counts; the result does not depend on how the
+    steps are split over calls (graph replays vs single launches), bit for bit."""
+    w = inputs.config2()
+    Xa, X0, p = gpu_steps(w, ds.F64, 101, tensor, integrator, t0=0.25)
+    Xb, _, _ = gpu_steps(w, ds.F64, 101, tensor, integrator, t0=0.25, chunks=[1, 33, 3, 64])
+    assert np.array_equal(Xa, Xb)
+    Xo = oracle.step(X0[0], w.phase[0], 0.25, 0, 101, p)
+    assert np.abs(Xa[0] - Xo).max() <= 1e-10 * ELL
+
+
+def test_step_zero_steps_and_state_errors():
+    w = inputs.config1()
+    s, _ = make_system(w, ds.F64)
+    with s:
+        buf = torch.empty((1, w.N, 3), dtype=torch.float64, device="cuda")
+        with pytest.raises(ds.DsError) as e:
+            s.step(1)
+        assert e.value.code == ds.ERR_STATE
+        with pytest.raises(ds.DsError):
+            s.get_state(buf)
+        s.set_state(dev(w.pos, ds.F64), torch.as_tensor(w.phase, device="cuda"))
+        s.step(0)
+        assert s.get_state(buf) == 0.0
+        assert np.array_equal(buf.cpu().numpy(), w.pos)
+        with pytest.raises(ds.DsError):
+            s.step(-1)
+    w5 = inputs.config5(B=2, S=4)
+    s, _ = make_system(w5, ds.F32)
+    with s:
+        s.set_state(dev(w5.pos, ds.F32), torch.as_tensor(w5.phase, device="cuda"))
+        with pytest.raises(ds.DsError) as e:
+            s.step(1)                      # ds_step requires n_batch == 1
+        assert e.value.code == ds.ERR_STATE
+        s.batch_step(2)
+
+
+def test_isolated_dumbbell_does_not_translate_on_gpu():
+    """PAPER.md:236 'single dumbbells did not translate' -- the authors' own acceptance check."""
+    phi = np.array([[0.9]])
+    n = np.array([[1.0, 2.0, -0.5]])
+    n /= np.linalg.norm(n)
+    X0 = inputs.place_spheres(np.array([[3.0, -1.0, 2.0]]), n, phi[0])[None]
+    w = inputs.Workload("single", X0, phi)
+    Xg, _, _ = gpu_steps(w, ds.F64, 3000)
+    assert np.abs(0.5 * (Xg[0, 0] + Xg[0, 1]) - np.array([3.0, -1.0, 2.0])).max() < 1e-12
