@@ -1,0 +1,462 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the hot path of arXiv 1004.1932 on B200, beside the CPU oracle.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--sweep]
+
+One bench "step" = one Heun time step of BASELINE.json config 4: a 3d random
+suspension of S = 2048 dumbbells (N = 4096 spheres), FP32 pair arithmetic, RPY tensor (the tensor
+the paper simulates with): force (Eq. 4) -> mobility apply (Eq. 3a,3b) -> predictor ->
+force -> mobility apply -> corrector, all on the device through ds_step (include/ds.h).
+Metric: ordered pair interactions per second, 2 N (N-1) per Heun step; timesteps/s is reported
+beside it for this and every other config.  The path does not shard: --gpus N runs N independent
+replicas, value = all replicas' pairs / the slowest replica's time.
+
+Prints ONE JSON line (rank 0).  `--impl reference` times the CPU oracle (oracle/) on the host
+cores instead; it is the only other place, with `cpu_baseline`, where this file runs oracle code.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "pair_interactions_per_s"
+UNIT = "pairs/s"
+# Algorithmic FLOP per ordered pair (FMA = 2, rsqrt not counted), DESIGN.md "FLOP count":
+FLOP_PER_PAIR = {"oseen": 27, "rpy": 33}
+# ALU peaks derived in DESIGN.md "Roofline": SMs x lanes x 2 x f_SM(max).  FP32: 128 lanes/SM.  FP64: the
+# DFMA rate of B200 is what ds_peak_probe measures; the nominal figure used is 64 lanes/SM.
+N_SM, F32_LANES, F64_LANES = 148, 128, 64
+
+
+def pairs_per_apply(N, B=1):
+    return B * N * (N - 1)
+
+
+# ----------------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """Samples SM clock, power and throttle reasons of one GPU through NVML while a timed region runs."""
+
+    def __init__(self, index, period=0.01):
+        self.index, self.period = index, period
+        self.sm, self.power, self.reasons = [], [], 0
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            try:  # CUDA ordinal -> NVML handle through the UUID (CUDA_VISIBLE_DEVICES may renumber)
+                import torch
+                self.h = pynvml.nvmlDeviceGetHandleByUUID("GPU-" + str(torch.cuda.get_device_properties(index).uuid))
+            except Exception:
+                self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception as e:  # no NVML: report that, never invent numbers
+            self.nv, self.err = None, repr(e)
+
+    def _run(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.sm.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+                self.reasons |= int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *exc):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self):
+        if self.nv is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml_unavailable"]}
+        names = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+                 0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+                 0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
+        reasons = [n for bit, n in names.items() if self.reasons & bit and n != "gpu_idle"]
+        return {"sm_mhz": float(np.median(self.sm)) if self.sm else None, "sm_max_mhz": self.max_mhz,
+                "reasons": reasons, "samples": len(self.sm),
+                "power_w_max": max(self.power) if self.power else None}
+
+
+# ----------------------------------------------------------------------------------------- GPU legs
+def _events(torch):
+    return torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+
+def time_steps(torch, ds, w, precision, tensor, n_steps, warmup, ranks=None, sampler=None):
+    """Device time of n_steps Heun steps of workload w through ds_step/ds_batch_step, state resident in
+    HBM.  Returns (seconds, launches in the timed region)."""
+    npdt = np.float32 if precision == ds.F32 else np.float64
+    stream = torch.cuda.current_stream()
+    sc = w.scalars
+    with ds.System(w.S, n_batch=w.B, precision=precision, tensor=tensor, integrator=ds.HEUN, a=sc["a"], eta=sc["eta"],
+                   ell=sc["ell"], lam=sc["lam"], omega=sc["omega"], k0=sc["k0"], dt=sc["dt"],
+                   device=torch.cuda.current_device(), stream=stream.cuda_stream) as s:
+        pos = torch.as_tensor(np.ascontiguousarray(w.pos, dtype=npdt), device="cuda")
+        phase = torch.as_tensor(w.phase, device="cuda")
+        s.set_state(pos, phase, 0.0)
+        step = s.batch_step if w.B > 1 else s.step
+        step(max(int(warmup), 0))
+        torch.cuda.synchronize()
+        e0, e1 = _events(torch)
+        if ranks is not None:
+            ranks.barrier()
+        torch.cuda.synchronize()
+        l0 = s.launch_count()
+        if sampler is not None:
+            sampler.__enter__()
+        e0.record(stream)
+        step(int(n_steps))
+        e1.record(stream)
+        torch.cuda.synchronize()
+        if sampler is not None:
+            sampler.__exit__()
+        if ranks is not None:
+            ranks.barrier()
+        out = torch.empty_like(pos)
+        s.get_state(out)
+        torch.cuda.synchronize()
+        if not bool(torch.isfinite(out).all()):
+            raise RuntimeError("non-finite state after the timed steps")
+        return e0.elapsed_time(e1) * 1e-3, s.launch_count() - l0
+
+
+def time_steps_cold_l2(torch, ds, w, precision, tensor, n_steps):
+    """Same step, one at a time, with L2 flushed (a 512 MiB write) before each: per-step device time."""
+    npdt = np.float32 if precision == ds.F32 else np.float64
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
+    with ds.System(w.S, n_batch=w.B, precision=precision, tensor=tensor, device=torch.cuda.current_device(),
+                   stream=stream.cuda_stream) as s:
+        pos = torch.as_tensor(np.ascontiguousarray(w.pos, dtype=npdt), device="cuda")
+        s.set_state(pos, torch.as_tensor(w.phase, device="cuda"), 0.0)
+        s.batch_step(3)
+        tot = 0.0
+        for _ in range(n_steps):
+            flush.fill_(1)
+            e0, e1 = _events(torch)
+            e0.record(stream)
+            s.batch_step(1)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            tot += e0.elapsed_time(e1) * 1e-3
+        return tot / n_steps
+
+
+def time_e2e(torch, ds, w, precision, tensor, n_steps, warmup, ranks=None):
+    """The same step through the C ABI with HOST buffers: every step copies the positions and phases
+    from pinned host memory to the device (ds_set_state), advances one Heun step (ds_step) and reads
+    the positions back to pinned host memory (ds_get_state).  Wall clock, synchronised on both sides."""
+    tdt = torch.float32 if precision == ds.F32 else torch.float64
+    npdt = np.float32 if precision == ds.F32 else np.float64
+    stream = torch.cuda.current_stream()
+    pos = torch.as_tensor(np.ascontiguousarray(w.pos, dtype=npdt)).pin_memory()
+    phase = torch.as_tensor(w.phase).pin_memory()
+    assert pos.dtype == tdt and not pos.is_cuda
+    h2d = pos.numel() * pos.element_size() + phase.numel() * phase.element_size()
+    d2h = pos.numel() * pos.element_size()
+    with ds.System(w.S, n_batch=w.B, precision=precision, tensor=tensor, device=torch.cuda.current_device(),
+                   stream=stream.cuda_stream) as s:
+        def one(k):
+            s.set_state(pos, phase, k * w.scalars["dt"])
+            s.batch_step(1)
+            s.get_state(pos)          # host pointer: synchronises the stream before returning
+        for k in range(max(int(warmup), 3)):
+            one(k)
+        torch.cuda.synchronize()
+        if ranks is not None:
+            ranks.barrier()
+        l0 = s.launch_count()
+        t0 = time.perf_counter()
+        for k in range(n_steps):
+            one(k)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        if ranks is not None:
+            ranks.barrier()
+        if not bool(torch.isfinite(pos).all()):
+            raise RuntimeError("non-finite state in the e2e loop")
+        return dt, h2d, d2h, s.launch_count() - l0
+
+
+def time_apply(torch, ds, N, precision, tensor, X, F, reps):
+    """Standalone ds_mobility_apply (a2 + a3 with arbitrary F), device buffers, `reps` back-to-back
+    launches replayed from a CUDA graph so that host launch cost does not enter.  Seconds per apply."""
+    npdt = np.float32 if precision == ds.F32 else np.float64
+    side = torch.cuda.Stream()
+    Xd = torch.as_tensor(np.ascontiguousarray(X, dtype=npdt), device="cuda")
+    Fd = torch.as_tensor(np.ascontiguousarray(F, dtype=npdt), device="cuda")
+    ud = torch.empty_like(Xd)
+    with ds.System(1, precision=precision, tensor=tensor, device=torch.cuda.current_device(),
+                   stream=side.cuda_stream) as s:
+        s.mobility_apply(Xd, Fd, ud, N)     # allocates the scratch outside the capture
+        side.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            s.set_stream(torch.cuda.current_stream().cuda_stream)
+            for _ in range(reps):
+                s.mobility_apply(Xd, Fd, ud, N)
+        s.set_stream(side.cuda_stream)
+        for _ in range(3):
+            g.replay()
+        torch.cuda.synchronize()
+        best = float("inf")
+        for _ in range(5):
+            e0, e1 = _events(torch)
+            e0.record()
+            g.replay()
+            e1.record()
+            torch.cuda.synchronize()
+            best = min(best, e0.elapsed_time(e1) * 1e-3 / reps)
+        if not bool(torch.isfinite(ud).all()):
+            raise RuntimeError("non-finite apply output")
+        del g
+        return best
+
+
+def peak_probe(ds, torch):
+    """Measured FMA-chain peaks (TFLOP/s) of this GPU: FP32 (packed FFMA2), FP64 (DFMA)."""
+    out = {}
+    try:
+        for name, prec in (("f32", ds.F32), ("f64", ds.F64)):
+            out[name + "_tflops"] = ds.peak_probe(prec, torch.cuda.current_device()) * 1e-12
+    except AttributeError:
+        return None
+    return out
+
+
+# ----------------------------------------------------------------------------------------- CPU legs
+def oracle_steps(w, tensor_name, n_steps, threads):
+    """Times the oracle, as it stands, on n_steps Heun steps of w (first system).  Returns seconds."""
+    import oracle
+    oracle.set_threads(threads)
+    sc = w.scalars
+    p = oracle.Params(a=sc["a"], eta=sc["eta"], ell=sc["ell"], lam=sc["lam"], omega=sc["omega"], k0=sc["k0"],
+                      dt=sc["dt"], tensor=oracle.RPY if tensor_name == "rpy" else oracle.OSEEN, integrator=oracle.HEUN)
+    X0 = np.asarray(w.pos[0], dtype=np.float32).astype(np.float64)
+    t0 = time.perf_counter()
+    X = oracle.step(X0, w.phase[0], 0.0, 0, n_steps, p)
+    dt = time.perf_counter() - t0
+    assert np.isfinite(X).all()
+    return dt
+
+
+def run_reference(args, ranks):
+    """--impl reference: the oracle on the host cores, same config/metric/unit; rank 0 only."""
+    if ranks.rank != 0:
+        return
+    import oracle
+    from paper_1004_1932_b200 import inputs
+    w = inputs.config4()
+    cores = oracle.max_threads()
+    N = w.N
+    for _ in range(min(args.warmup, 1)):
+        oracle_steps(w, args.tensor, 1, cores)
+    per = []
+    for _ in range(args.steps):
+        per.append(oracle_steps(w, args.tensor, 1, cores))
+    tot = sum(per)
+    value = args.steps * 2 * pairs_per_apply(N) / tot
+    sample = f"{args.steps} x 1 Heun step of C4 (N={N}), fp64 oracle, OpenMP over alpha on {cores} threads"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(w, args, "f64"),
+            "timesteps_per_s": args.steps / tot,
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(w, args, dtype):
+    return {"workload": f"BASELINE.json configs[3]: 3d random suspension S={w.S} dumbbells (N={w.N} spheres), "
+                        f"density 1/(4 ell)^3, hard core 2.5a, seed {w.seed}; one step = one Heun time step "
+                        f"(2 mobility applies + forces + predictor/corrector)",
+            "N": w.N, "S": w.S, "B": w.B, "tensor": args.tensor, "precision": dtype, "integrator": "heun",
+            "dt": w.scalars["dt"], "k0": w.scalars["k0"],
+            "pairs_per_step": 2 * pairs_per_apply(w.N, w.B), "flop_per_pair": FLOP_PER_PAIR[args.tensor],
+            "parallelism": f"replicas x{args.gpus}" if args.gpus > 1 else "single GPU",
+            "l2": "warm by construction: the 256 KB state is produced on the device by the previous step and "
+                  "never leaves it (the method has no host round trip per step); the cold-L2 per-step figure "
+                  "(512 MiB flush before every step) is in extra.cold_l2"}
+
+
+def extras(torch, ds, inputs, w, args, precision, tensor):
+    """Beside the headline: the standalone apply at N = 4096 (4 variants), timesteps/s of every config,
+    the cold-L2 per-step figure, and (with --sweep) the N = 256 .. 65536 apply sweep."""
+    extra = {}
+    # apply at N = 4096, all four variants (the standalone sweep of config 4)
+    Xa, Fa = inputs.apply_case(4096, 1004, 2004)
+    ap = {}
+    for pname, pr in (("f32", ds.F32), ("f64", ds.F64)):
+        for tname, tn in (("oseen", ds.OSEEN), ("rpy", ds.RPY)):
+            t = time_apply(torch, ds, 4096, pr, tn, Xa, Fa, reps=200)
+            ln = F32_LANES if pname == "f32" else F64_LANES
+            ap[f"{pname}_{tname}"] = {"us": t * 1e6, "pairs_per_s": pairs_per_apply(4096) / t,
+                                      "frac_of_alu_peak": pairs_per_apply(4096) * FLOP_PER_PAIR[tname] / t /
+                                      (N_SM * ln * 2 * 1.965e9)}
+    extra["apply_N4096"] = ap
+    # timesteps/s for every config
+    cfgs = {}
+    for name, mk, pr, nst in (("C1_N16_f64", inputs.config1, ds.F64, 10_000),
+                              ("C2_N128_f32", inputs.config2, ds.F32, 10_000),
+                              ("C2_N128_f64", inputs.config2, ds.F64, 10_000),
+                              ("C3_N1024_f32", inputs.config3, ds.F32, 10_000),
+                              ("C4_N4096_f32", inputs.config4, ds.F32, 1000),
+                              ("C4_N4096_f64", inputs.config4, ds.F64, 1000),
+                              ("C5_B64_N512_f32", inputs.config5, ds.F32, 2000)):
+        wc = w if mk is inputs.config4 else mk()
+        t, _ = time_steps(torch, ds, wc, pr, ds.RPY, nst, 64)
+        cfgs[name] = {"timesteps_per_s": nst / t, "pairs_per_s": nst * 2 * pairs_per_apply(wc.N, wc.B) / t,
+                      "steps_timed": nst}
+    extra["configs_rpy_heun"] = cfgs
+    extra["cold_l2"] = {"ms_per_step": 1e3 * time_steps_cold_l2(torch, ds, w, precision, tensor, 30),
+                        "steps": 30, "flush": "512 MiB fill before every step"}
+    if args.sweep:
+        sw = {}
+        for lg in range(8, 17):
+            Xs, Fs = inputs.sweep_case(lg)
+            n = 1 << lg
+            for tname, tn in (("oseen", ds.OSEEN), ("rpy", ds.RPY)):
+                reps = max(2, min(200, int(2e10 / (n * n))))
+                t = time_apply(torch, ds, n, ds.F32, tn, Xs, Fs, reps=reps)
+                sw[f"N{n}_{tname}"] = {"us": t * 1e6, "pairs_per_s": pairs_per_apply(n) / t,
+                                       "frac_of_alu_peak": pairs_per_apply(n) * FLOP_PER_PAIR[tname] / t /
+                                       (N_SM * F32_LANES * 2 * 1.965e9)}
+        extra["sweep_f32"] = sw
+    return extra
+
+
+# ----------------------------------------------------------------------------------------- main
+def run_ours(args, ranks):
+    import torch
+    from paper_1004_1932_b200 import ds, inputs
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback "
+                         "(use --impl reference for the CPU oracle)")
+    torch.cuda.set_device(ranks.local_rank)
+    ds.lib()  # fails loudly if libds.so cannot be built / loaded
+    precision = ds.F32 if args.precision == "f32" else ds.F64
+    tensor = ds.RPY if args.tensor == "rpy" else ds.OSEEN
+    w = inputs.config4()
+    N = w.N
+    flop_pair = FLOP_PER_PAIR[args.tensor]
+
+    # ---- the timed region: K Heun steps, state resident in HBM ----
+    sampler = ClockSampler(torch.cuda.current_device())
+    sec, launches = time_steps(torch, ds, w, precision, tensor, args.steps, max(args.warmup, 3), ranks, sampler)
+    clocks = sampler.summary()
+    sec_max = ranks.max(sec)
+    pairs_step = 2 * pairs_per_apply(N)
+    value = ranks.sum(args.steps * pairs_step) / sec_max
+
+    # ---- e2e through host buffers ----
+    e_sec, h2d, d2h, e_launches = time_e2e(torch, ds, w, precision, tensor, args.steps, args.warmup, ranks)
+    e_value = ranks.sum(args.steps * pairs_step) / ranks.max(e_sec)
+
+    line = None
+    if ranks.rank == 0:
+        kernel_s = sec / (2 * args.steps)          # two mobility launches per Heun step, nothing else
+        lanes = F32_LANES if args.precision == "f32" else F64_LANES
+        peak_nominal = N_SM * lanes * 2 * 1.965e9 * 1e-12
+        achieved = pairs_per_apply(N) * flop_pair / kernel_s * 1e-12
+        roof = {"bound": "alu", "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s",
+                "frac": achieved / peak_nominal, "traffic": None,
+                "kernel": "ds::mobility_kernel (pair sum + fused split-j reduce + Heun epilogue + next forces)",
+                "kernel_us": kernel_s * 1e6, "launches_per_step": 2,
+                "peak_kind": f"derived: {N_SM} SMs x {lanes} {args.precision} FMA lanes x 2 x 1.965 GHz "
+                             f"(MEASURED_PEAKS.json sm_max_mhz); MEASURED_PEAKS.json has no ALU entry",
+                "flop_per_pair": flop_pair, "pairs_per_launch": pairs_per_apply(N)}
+        if clocks.get("sm_mhz"):
+            roof["frac_at_sampled_clock"] = achieved / (N_SM * lanes * 2 * clocks["sm_mhz"] * 1e6 * 1e-12)
+        probe = peak_probe(ds, torch)
+        if probe:
+            roof["measured_fma_chain"] = probe
+            roof["frac_of_measured_chain"] = achieved / probe[args.precision + "_tflops"]
+
+        extra = None if args.quick else extras(torch, ds, inputs, w, args, precision, tensor)
+
+        # ---- the oracle beside it (bounded sample) ----
+        import oracle
+        cores = oracle.max_threads()
+        n_or = 1 if args.quick else args.cpu_steps
+        oracle_steps(w, args.tensor, 1, cores)
+        t_or = oracle_steps(w, args.tensor, n_or, cores)
+        t_or1 = oracle_steps(w, args.tensor, 1, 1)
+        cpu = {"value": n_or * pairs_step / t_or, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"{n_or} Heun steps of the same C4 workload (N={N}), fp64, OpenMP over alpha",
+               "timesteps_per_s": n_or / t_or,
+               "single_thread": {"value": pairs_step / t_or1, "unit": UNIT, "cores": 1, "sample": "1 Heun step"}}
+
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+                "warmup": max(args.warmup, 3), "ms_per_step": 1e3 * sec_max / args.steps, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": args.precision, "data": "synthetic",
+                "config": workload_config(w, args, args.precision),
+                "timesteps_per_s": args.steps / sec_max,
+                "clocks": clocks,
+                "e2e": {"value": e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                        "ms_per_step": 1e3 * e_sec / args.steps,
+                        "path": "ds_set_state(host pos, host phase) + ds_step(1) + ds_get_state(host pos), pinned"},
+                "gpu_launches": int(launches),
+                "roofline": roof, "cpu_baseline": cpu, "extra": extra}
+    ranks.barrier()
+    if line is not None:
+        print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--precision", choices=["f32", "f64"], default="f32")
+    ap.add_argument("--tensor", choices=["oseen", "rpy"], default="rpy")
+    ap.add_argument("--cpu-steps", type=int, default=20, help="oracle Heun steps timed for cpu_baseline")
+    ap.add_argument("--sweep", action="store_true", help="add the N = 256 .. 65536 apply sweep to extra")
+    ap.add_argument("--quick", action="store_true", help="headline + e2e only (used under ncu)")
+    args = ap.parse_args()
+    ref = args.impl == "reference"
+    if args.steps is None:
+        args.steps = 10 if ref else 4000
+    if args.warmup is None:
+        args.warmup = 1 if ref else 200
+    from paper_1004_1932_b200.replicas import Ranks
+    if ref:
+        # rank 0 alone runs the oracle; the other ranks exit 0 without work (no process group needed)
+        class _R:
+            rank = int(os.environ.get("RANK", "0"))
+        run_reference(args, _R())
+        return
+    ranks = Ranks()
+    if ranks.world != args.gpus:
+        raise SystemExit(f"--gpus {args.gpus} but WORLD_SIZE={ranks.world}: launch with torch.distributed.run "
+                         f"--nproc-per-node {args.gpus}")
+    try:
+        run_ours(args, ranks)
+    finally:
+        ranks.close()
+
+
+if __name__ == "__main__":
+    main()

@@ -127,6 +127,11 @@ int ds_set_tuning(ds_system *s, int32_t j_splits);
 /* Number of kernels launched by this system since creation (bench.py's gpu_launches claim). */
 int64_t ds_launch_count(const ds_system *s);
 
+/* Measurement aid for the roofline denominators (bench.py): runs an FMA-chain microbenchmark on
+ * `device` (packed FP32 FMA for DS_F32, DFMA for DS_F64) and writes the best achieved FLOP/s
+ * (FMA = 2) to *flops_per_s (HOST pointer).  Synchronous; uses the legacy default stream.       */
+int ds_peak_probe(int32_t precision, int32_t device, double *flops_per_s);
+
 const char *ds_strerror(int code);
 const char *ds_last_cuda_error(void); /* text of the last failing CUDA call on this thread, or "" */
 const char *ds_version(void);

@@ -12,6 +12,7 @@
 
 #include "../../include/ds.h"
 #include "mobility.cuh"
+#include "peak.cuh"
 #include "state.cuh"
 
 namespace {
@@ -281,6 +282,31 @@ template <typename T> int run_pad_init(ds_system *s, void *p4, void *f4) {
     ds::pad_init_kernel<T><<<(unsigned)((n + 127) / 128), 128, 0, s->stream>>>(p4, f4, s->N, s->Npad, s->B);
     CU_TRY(cudaGetLastError());
     s->launches += 1;
+    return DS_OK;
+}
+
+template <typename T> int peak_probe_t(int num_sms, double *flops_per_s) {
+    constexpr int CHAINS = 12, THREADS = 256, ITERS = 2048;
+    const int blocks = num_sms * 8;
+    T *out = nullptr;
+    CU_TRY(cudaMalloc((void **)&out, (size_t)blocks * THREADS * sizeof(T)));
+    cudaEvent_t e0, e1;
+    CU_TRY(cudaEventCreate(&e0));
+    CU_TRY(cudaEventCreate(&e1));
+    float best_ms = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {  // rep 0 warms up
+        CU_TRY(cudaEventRecord(e0, 0));
+        ds::fma_chain_kernel<T, CHAINS><<<blocks, THREADS>>>(out, ITERS, (T)0.999, (T)0.001);
+        CU_TRY(cudaEventRecord(e1, 0));
+        CU_TRY(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        CU_TRY(cudaEventElapsedTime(&ms, e0, e1));
+        if (rep > 0 && ms < best_ms) best_ms = ms;
+    }
+    CU_TRY(cudaGetLastError());
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(out);
+    const double flops = (double)blocks * THREADS * ITERS * 8.0 * CHAINS * ds::Pack<T>::W * 2.0;
+    *flops_per_s = flops / (best_ms * 1e-3);
     return DS_OK;
 }
 
@@ -558,6 +584,20 @@ int ds_batch_step(ds_system *s, int64_t n_steps) {
         s->n_host += 1; left -= 1;
     }
     return DS_OK;
+}
+
+int ds_peak_probe(int32_t precision, int32_t device, double *flops_per_s) {
+    if (!flops_per_s) return DS_ERR_NULL;
+    if (precision != DS_F32 && precision != DS_F64) return DS_ERR_INVALID_PARAM;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { (void)cudaGetLastError(); return DS_ERR_NO_DEVICE; }
+    if (device < 0 || device >= ndev) return DS_ERR_INVALID_PARAM;
+    cudaDeviceProp prop;
+    CU_TRY(cudaGetDeviceProperties(&prop, device));
+    if (prop.major != 10) return DS_ERR_NO_DEVICE;
+    CU_TRY(cudaSetDevice(device));
+    return precision == DS_F64 ? peak_probe_t<double>(prop.multiProcessorCount, flops_per_s)
+                               : peak_probe_t<float>(prop.multiProcessorCount, flops_per_s);
 }
 
 int ds_step(ds_system *s, int64_t n_steps) {

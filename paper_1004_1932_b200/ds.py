@@ -23,7 +23,7 @@ ERR_INVALID_PARAM, ERR_NULL, ERR_CUDA, ERR_STATE, ERR_NO_DEVICE, ERR_ALLOC = -1,
 # every symbol include/ds.h declares (tests check that the built library exports all of them)
 SYMBOLS = ["ds_create", "ds_destroy", "ds_set_stream", "ds_set_state", "ds_get_state", "ds_forces",
            "ds_mobility_apply", "ds_step", "ds_batch_step", "ds_velocity", "ds_set_tuning", "ds_launch_count",
-           "ds_strerror", "ds_last_cuda_error", "ds_version"]
+           "ds_peak_probe", "ds_strerror", "ds_last_cuda_error", "ds_version"]
 
 
 class DsError(RuntimeError):
@@ -67,6 +67,7 @@ def lib():
         L.ds_set_tuning.argtypes = [vp, i32]
         L.ds_launch_count.argtypes = [vp]
         L.ds_launch_count.restype = i64
+        L.ds_peak_probe.argtypes = [i32, i32, ctypes.POINTER(dbl)]
         for f in ("ds_strerror", "ds_last_cuda_error", "ds_version"):
             getattr(L, f).restype = ctypes.c_char_p
         L.ds_strerror.argtypes = [ctypes.c_int]
@@ -76,6 +77,13 @@ def lib():
 
 def version():
     return lib().ds_version().decode()
+
+
+def peak_probe(precision, device=0):
+    """Measured FMA-chain peak of `device` in FLOP/s (FMA = 2)."""
+    v = ctypes.c_double()
+    _check(lib().ds_peak_probe(int(precision), int(device), ctypes.byref(v)), "ds_peak_probe")
+    return v.value
 
 
 def _ptr(x):
