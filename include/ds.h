@@ -121,8 +121,9 @@ int ds_batch_step(ds_system *s, int64_t n_steps);
  * right-hand side of Eq. (1a) the integrator uses; exported for tests and observables).        */
 int ds_velocity(ds_system *s, void *V);
 
-/* Launch-shape override for tuning and tests: number of j-splits (0 = library heuristic). */
-int ds_set_tuning(ds_system *s, int32_t j_splits);
+/* Launch-shape override for tuning and tests: number of row tiles (CTAs) per system; 0 = library
+ * heuristic.  Values below ceil(ceil(N/4)/512) or above ceil(N/4) are clamped.                   */
+int ds_set_tuning(ds_system *s, int32_t n_tiles);
 
 /* Number of kernels launched by this system since creation (bench.py's gpu_launches claim). */
 int64_t ds_launch_count(const ds_system *s);

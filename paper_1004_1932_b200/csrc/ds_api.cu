@@ -36,21 +36,7 @@ thread_local char g_cuda_err[512] = "";
         if (r_ != DS_OK) return r_; \
     } while (0)
 
-// ---- kernel shape (compile-time) -------------------------------------------------------------
-// FP32: 4 alpha per lane x 2 beta per pack; FP64: 2 alpha per lane.  See DESIGN.md "Kernels".
-struct ShapeF32 { static constexpr int I = 4, WI = 2, WJ = 4, SJ = 1024, UNROLL = 2, MINB = 2; };
-struct ShapeF64 { static constexpr int I = 2, WI = 4, WJ = 2, SJ = 1024, UNROLL = 2, MINB = 2; };
-template <typename T> struct ShapeOf;
-template <> struct ShapeOf<float> { typedef ShapeF32 S; };
-template <> struct ShapeOf<double> { typedef ShapeF64 S; };
-
-template <typename T> constexpr int tile_i() { return 32 * ShapeOf<T>::S::I * ShapeOf<T>::S::WI; }
-template <typename T> constexpr int group_j() { return ds::Pack<T>::W * ShapeOf<T>::S::WJ; }
-template <typename T> constexpr size_t smem_bytes() {
-    typedef typename ShapeOf<T>::S S;
-    return ds::stage_bytes_for<T>(S::SJ) + (size_t)S::WJ * 3 * tile_i<T>() * sizeof(double) +
-           (size_t)2 * 3 * tile_i<T>() * sizeof(double);
-}
+template <typename T> constexpr int pack_w() { return ds::Pack<T>::W; }
 
 struct Buf {
     void *p = nullptr;
@@ -64,26 +50,25 @@ struct ds_system {
     cudaStream_t stream = nullptr;
     cudaStream_t cap_stream = nullptr;
     int num_sms = 148;
-    int N = 0, B = 0, S = 0, Npad = 0, n_it = 0;
-    int tune_js = 0;
+    int N = 0, B = 0, S = 0;
+    int W = 1;                  // spheres per unit: 2 (FP32 packs) or 1 (FP64)
+    int NQ = 0, U = 0;          // quads = ceil(N/4), units = ceil(N/W)
+    long long unit_stride = 0;  // units per system in the streams
+    int tune_cta = 0, n_cta = 1;
     bool has_state = false;
     double t0 = 0.0;
     long long n_host = 0;  // mirror of the device step counter
     int64_t launches = 0;
     // state
     double *X = nullptr, *V1 = nullptr, *FdA = nullptr, *FdB = nullptr, *phase = nullptr;
-    void *pos4A = nullptr, *F4A = nullptr, *pos4B = nullptr, *F4B = nullptr;
-    double *partial = nullptr;
-    unsigned *counters = nullptr;
-    long long *stepc = nullptr;  // c[0], c[1]
-    int JS = 1, jchunk = 0;
+    void *unitsA = nullptr, *unitsB = nullptr;  // beta-streams (mobility.cuh), ping-pong
+    long long *stepc = nullptr;                 // c[0], c[1]
     // graphs
     cudaGraphExec_t graphK = nullptr;  // GRAPH_STEPS steps
     int graph_steps = 0;
     int graph_nodes = 0;
     // scratch of the stateless apply and of host-pointer staging
-    Buf ap_partial, ap_counters, st_a, st_b, st_c;
-    int ap_counters_n = 0;
+    Buf ap_units, st_a, st_b, st_c;
 };
 
 namespace {
@@ -116,56 +101,51 @@ int is_device_ptr(const void *p, int *out) {
 
 size_t elem_size(const ds_system *s) { return s->P.precision == DS_F64 ? sizeof(double) : sizeof(float); }
 
-// Launch shape: JS j-splits of jchunk spheres so that B*n_it*JS blocks fill the SMs in whole waves.
-void choose_split(const ds_system *s, int N, int B, int n_it, int gj, int resident_per_sm, int *JS, int *jchunk) {
-    const int slots = s->num_sms * resident_per_sm;
-    const long long tiles = (long long)B * n_it;
-    const int min_chunk = 16 * gj;  // at least 16 inner iterations per j-warp-group
-    int js_max = (N + min_chunk - 1) / min_chunk;
-    if (js_max < 1) js_max = 1;
-    int best = 1;
-    if (s->tune_js > 0) {
-        best = s->tune_js < js_max ? s->tune_js : js_max;
-    } else {
-        double best_cost = 1e300;
-        for (int js = 1; js <= js_max && js <= 4096; ++js) {
-            const int ch = ((N + js - 1) / js + gj - 1) / gj * gj;
-            const int js_eff = (N + ch - 1) / ch;
-            const long long ctas = tiles * js_eff;
-            const long long waves = (ctas + slots - 1) / slots;
-            // time ~ waves * (chunk + fixed per-block overhead expressed in j-iterations)
-            const double cost = (double)waves * ((double)ch + 48.0) + 0.02 * js_eff;
-            if (cost < best_cost) { best_cost = cost; best = js_eff; }
-        }
+// Launch shape: n_cta row tiles per system (mobility.cuh).  Every CTA walks all U units with
+// n_jg = NT / nq beta-groups, i.e. ceil(U / n_jg) iterations of 4 alpha x 1 unit per thread, so the
+// modelled time of a launch is waves x (iterations + a fixed per-CTA cost, in iterations).
+int choose_tiles(const ds_system *s, int NQ, int U, int B) {
+    const int lo = (NQ + ds::NT - 1) / ds::NT;  // nq <= NT
+    if (s->tune_cta > 0) {
+        int t = s->tune_cta < lo ? lo : s->tune_cta;
+        return t > NQ ? NQ : t;
     }
-    int ch = ((N + best - 1) / best + gj - 1) / gj * gj;
-    *jchunk = ch;
-    *JS = (N + ch - 1) / ch;
+    const int hi = NQ < 16 * s->num_sms ? NQ : 16 * s->num_sms;
+    double best_cost = 1e300;
+    int best = lo;
+    for (int n = lo; n <= hi; ++n) {
+        const int nq = (NQ + n - 1) / n;
+        const int n_jg = ds::NT / nq;
+        const long long iters = (U + n_jg - 1) / n_jg;
+        const long long waves = ((long long)B * n + s->num_sms - 1) / s->num_sms;
+        const double cost = (double)waves * ((double)iters + 6.0);
+        if (cost < best_cost * (1.0 - 1e-9)) { best_cost = cost; best = n; }
+    }
+    return best;
 }
 
-template <typename T, int TENSOR, bool USER> int launch_mob_t(ds_system *s, const ds::MobArgs &A, cudaStream_t st) {
-    typedef typename ShapeOf<T>::S S;
-    auto kern = ds::mobility_kernel<T, TENSOR, USER, S::I, S::WI, S::WJ, S::SJ, S::UNROLL, S::MINB>;
+template <typename T, int TENSOR> int launch_mob_t(ds_system *s, const ds::MobArgs &A, cudaStream_t st) {
+    auto kern = ds::mobility_kernel<T, TENSOR>;
     static bool attr_done = false;
     if (!attr_done) {
-        CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<T>()));
+        CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, ds::SMEM_BYTES));
         attr_done = true;
     }
-    dim3 grid((unsigned)A.JS, (unsigned)A.n_it, (unsigned)A.B), block(32 * S::WI * S::WJ);
-    kern<<<grid, block, smem_bytes<T>(), st>>>(A);
+    dim3 grid((unsigned)A.n_cta, (unsigned)A.B), block(ds::NT);
+    kern<<<grid, block, ds::SMEM_BYTES, st>>>(A);
     CU_TRY(cudaGetLastError());
     s->launches += 1;
     return DS_OK;
 }
 
-int launch_mob(ds_system *s, const ds::MobArgs &A, bool user, cudaStream_t st) {
+int launch_mob(ds_system *s, const ds::MobArgs &A, cudaStream_t st) {
     const bool f64 = s->P.precision == DS_F64, rpy = s->P.tensor == DS_RPY;
-    if (f64) {
-        if (rpy) return user ? launch_mob_t<double, ds::TENSOR_RPY, true>(s, A, st) : launch_mob_t<double, ds::TENSOR_RPY, false>(s, A, st);
-        return user ? launch_mob_t<double, ds::TENSOR_OSEEN, true>(s, A, st) : launch_mob_t<double, ds::TENSOR_OSEEN, false>(s, A, st);
-    }
-    if (rpy) return user ? launch_mob_t<float, ds::TENSOR_RPY, true>(s, A, st) : launch_mob_t<float, ds::TENSOR_RPY, false>(s, A, st);
-    return user ? launch_mob_t<float, ds::TENSOR_OSEEN, true>(s, A, st) : launch_mob_t<float, ds::TENSOR_OSEEN, false>(s, A, st);
+    if (f64) return rpy ? launch_mob_t<double, ds::TENSOR_RPY>(s, A, st) : launch_mob_t<double, ds::TENSOR_OSEEN>(s, A, st);
+    return rpy ? launch_mob_t<float, ds::TENSOR_RPY>(s, A, st) : launch_mob_t<float, ds::TENSOR_OSEEN>(s, A, st);
+}
+
+void fill_shape(const ds_system *s, ds::MobArgs &A) {
+    A.N = s->N; A.B = s->B; A.NQ = s->NQ; A.U = s->U; A.n_cta = s->n_cta; A.unit_stride = s->unit_stride;
 }
 
 void fill_constants(const ds_system *s, ds::MobArgs &A) {
@@ -177,30 +157,27 @@ void fill_constants(const ds_system *s, ds::MobArgs &A) {
     A.t0 = s->t0; A.dt = s->P.dt; A.ell = s->P.ell; A.lambda = s->P.lambda; A.omega = s->P.omega; A.k0 = s->P.k0;
 }
 
-// One stage of the integrator on the system's own state.  set 0: (pos4A,F4A,FdA) -> writes set B
+// One stage of the integrator on the system's own state.  set 0: (unitsA,FdA) -> writes set B
 // (predictor) ; set 1: reads B, writes A (corrector).  Euler reads A and writes A... see below.
 int launch_state_stage(ds_system *s, int mode, int cr, int cw, long long inc, cudaStream_t st) {
     ds::MobArgs A;
     memset(&A, 0, sizeof A);
-    A.N = s->N; A.B = s->B; A.Npad = s->Npad; A.n_it = s->n_it; A.JS = s->JS; A.jchunk = s->jchunk;
-    A.partial = s->partial; A.counters = s->counters;
+    fill_shape(s, A);
     fill_constants(s, A);
     A.mode = mode;
     A.X = s->X; A.V1 = s->V1; A.phase = s->phase;
     A.n_read = s->stepc + cr; A.n_write = s->stepc + cw; A.n_inc = inc;
     const bool fromB = (mode == ds::EPI_CORR);
-    A.src_pos = fromB ? s->pos4B : s->pos4A;
-    A.src_F = fromB ? s->F4B : s->F4A;
+    A.src_units = fromB ? s->unitsB : s->unitsA;
     A.Fd_in = fromB ? s->FdB : s->FdA;
     const bool toB = (mode == ds::EPI_PRED);
-    A.pos4_out = toB ? s->pos4B : s->pos4A;
-    A.F4_out = toB ? s->F4B : s->F4A;
+    A.units_out = toB ? s->unitsB : s->unitsA;
     A.Fd_out = toB ? s->FdB : s->FdA;
-    return launch_mob(s, A, false, st);
+    return launch_mob(s, A, st);
 }
 
 // One full step.  Heun: PRED (reads c[0], writes c[1] = n) then CORR (reads c[1], writes c[0] = n+1).
-// Euler: in place on set A is NOT safe (other blocks still read pos4A), so Euler ping-pongs the
+// Euler: in place on set A is NOT safe (other blocks still read unitsA), so Euler ping-pongs the
 // packed sets: even steps read A write B, odd steps read B write A; the counters ping-pong too.
 int launch_one_step(ds_system *s, long long n_index, cudaStream_t st) {
     if (s->P.integrator == DS_HEUN) {
@@ -210,15 +187,14 @@ int launch_one_step(ds_system *s, long long n_index, cudaStream_t st) {
     const int par = (int)(n_index & 1);
     ds::MobArgs A;
     memset(&A, 0, sizeof A);
-    A.N = s->N; A.B = s->B; A.Npad = s->Npad; A.n_it = s->n_it; A.JS = s->JS; A.jchunk = s->jchunk;
-    A.partial = s->partial; A.counters = s->counters;
+    fill_shape(s, A);
     fill_constants(s, A);
     A.mode = ds::EPI_EULER;
     A.X = s->X; A.V1 = s->V1; A.phase = s->phase;
     A.n_read = s->stepc + par; A.n_write = s->stepc + (par ^ 1); A.n_inc = 1;
-    A.src_pos = par ? s->pos4B : s->pos4A; A.src_F = par ? s->F4B : s->F4A; A.Fd_in = par ? s->FdB : s->FdA;
-    A.pos4_out = par ? s->pos4A : s->pos4B; A.F4_out = par ? s->F4A : s->F4B; A.Fd_out = par ? s->FdA : s->FdB;
-    return launch_mob(s, A, false, st);
+    A.src_units = par ? s->unitsB : s->unitsA; A.Fd_in = par ? s->FdB : s->FdA;
+    A.units_out = par ? s->unitsA : s->unitsB; A.Fd_out = par ? s->FdA : s->FdB;
+    return launch_mob(s, A, st);
 }
 
 void destroy_graphs(ds_system *s) {
@@ -253,7 +229,7 @@ int set_device(const ds_system *s) {
 template <typename T> int run_state_init(ds_system *s, const void *dpos) {
     ds::StateArgs A;
     memset(&A, 0, sizeof A);
-    A.N = s->N; A.B = s->B; A.Npad = s->Npad; A.user_pos = dpos; A.X = s->X; A.pos4 = s->pos4A; A.F4 = s->F4A;
+    A.N = s->N; A.B = s->B; A.unit_stride = s->unit_stride; A.user_pos = dpos; A.X = s->X; A.units = s->unitsA;
     A.Fd = s->FdA; A.phase = s->phase; A.counters = s->stepc; A.t = s->t0;
     A.ell = s->P.ell; A.lambda = s->P.lambda; A.omega = s->P.omega; A.k0 = s->P.k0;
     const long long n = (long long)s->B * s->S;
@@ -266,7 +242,7 @@ template <typename T> int run_state_init(ds_system *s, const void *dpos) {
 template <typename T> int run_forces_out(ds_system *s, void *dF) {
     ds::StateArgs A;
     memset(&A, 0, sizeof A);
-    A.N = s->N; A.B = s->B; A.Npad = s->Npad; A.user_out = dF; A.X = s->X; A.phase = s->phase;
+    A.N = s->N; A.B = s->B; A.unit_stride = s->unit_stride; A.user_out = dF; A.X = s->X; A.phase = s->phase;
     A.t = s->t0 + (double)s->n_host * s->P.dt;
     A.ell = s->P.ell; A.lambda = s->P.lambda; A.omega = s->P.omega; A.k0 = s->P.k0;
     const long long n = (long long)s->B * s->S;
@@ -276,10 +252,10 @@ template <typename T> int run_forces_out(ds_system *s, void *dF) {
     return DS_OK;
 }
 
-template <typename T> int run_pad_init(ds_system *s, void *p4, void *f4) {
-    const long long n = (long long)s->B * (s->Npad - s->N);
+template <typename T> int run_pad_init(ds_system *s, void *units) {
+    const long long n = (long long)s->B * (s->unit_stride - s->U);
     if (n <= 0) return DS_OK;
-    ds::pad_init_kernel<T><<<(unsigned)((n + 127) / 128), 128, 0, s->stream>>>(p4, f4, s->N, s->Npad, s->B);
+    ds::pad_init_kernel<T><<<(unsigned)((n + 127) / 128), 128, 0, s->stream>>>(units, s->U, s->unit_stride, s->B);
     CU_TRY(cudaGetLastError());
     s->launches += 1;
     return DS_OK;
@@ -362,27 +338,26 @@ int ds_create(const ds_params *p, ds_system **out) {
     s->num_sms = prop.multiProcessorCount;
     s->S = p->n_dumbbells; s->N = 2 * p->n_dumbbells; s->B = p->n_batch;
     const bool f64 = p->precision == DS_F64;
-    const int TI = f64 ? tile_i<double>() : tile_i<float>();
-    s->n_it = (s->N + TI - 1) / TI;
-    s->Npad = s->n_it * TI;
+    s->W = f64 ? pack_w<double>() : pack_w<float>();
+    s->NQ = (s->N + ds::QI - 1) / ds::QI;
+    s->U = (s->N + s->W - 1) / s->W;
+    s->unit_stride = (long long)s->U + ds::PAD_UNITS;
     int rc = DS_OK;
     auto fail = [&](int code) { ds_destroy(s); return code; };
     if (set_device(s) != DS_OK) return fail(DS_ERR_CUDA);
     if (cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking) != cudaSuccess) return fail(DS_ERR_CUDA);
-    const size_t n3 = (size_t)s->B * s->N * 3, np = (size_t)s->B * s->Npad;
-    const size_t t4 = f64 ? sizeof(double4) : sizeof(float4);
+    const size_t n3 = (size_t)s->B * s->N * 3;
+    const size_t ub = (size_t)s->B * (size_t)s->unit_stride * ds::UNIT_BYTES;
     cudaError_t e = cudaSuccess;
     auto al = [&](void **ptr, size_t bytes) { if (e == cudaSuccess) e = cudaMalloc(ptr, bytes); };
     al((void **)&s->X, n3 * 8); al((void **)&s->V1, n3 * 8); al((void **)&s->FdA, n3 * 8); al((void **)&s->FdB, n3 * 8);
     al((void **)&s->phase, (size_t)s->B * s->S * 8);
-    al(&s->pos4A, np * t4); al(&s->F4A, np * t4); al(&s->pos4B, np * t4); al(&s->F4B, np * t4);
-    al((void **)&s->counters, (size_t)s->B * s->n_it * sizeof(unsigned));
+    al(&s->unitsA, ub); al(&s->unitsB, ub);
     al((void **)&s->stepc, 2 * sizeof(long long));
     if (e != cudaSuccess) { snprintf(g_cuda_err, sizeof g_cuda_err, "cudaMalloc -> %s", cudaGetErrorString(e)); (void)cudaGetLastError(); return fail(DS_ERR_ALLOC); }
-    if (cudaMemset(s->counters, 0, (size_t)s->B * s->n_it * sizeof(unsigned)) != cudaSuccess) return fail(DS_ERR_CUDA);
     if (cudaMemset(s->stepc, 0, 2 * sizeof(long long)) != cudaSuccess) return fail(DS_ERR_CUDA);
-    rc = f64 ? run_pad_init<double>(s, s->pos4A, s->F4A) : run_pad_init<float>(s, s->pos4A, s->F4A);
-    if (rc == DS_OK) rc = f64 ? run_pad_init<double>(s, s->pos4B, s->F4B) : run_pad_init<float>(s, s->pos4B, s->F4B);
+    rc = f64 ? run_pad_init<double>(s, s->unitsA) : run_pad_init<float>(s, s->unitsA);
+    if (rc == DS_OK) rc = f64 ? run_pad_init<double>(s, s->unitsB) : run_pad_init<float>(s, s->unitsB);
     if (rc != DS_OK) return fail(rc);
     rc = ds_set_tuning(s, 0);
     if (rc != DS_OK) return fail(rc);
@@ -397,8 +372,8 @@ int ds_destroy(ds_system *s) {
     cudaStreamSynchronize(s->stream);
     destroy_graphs(s);
     if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
-    void *ptrs[] = {s->X, s->V1, s->FdA, s->FdB, s->phase, s->pos4A, s->F4A, s->pos4B, s->F4B, s->partial,
-                    s->counters, s->stepc, s->ap_partial.p, s->ap_counters.p, s->st_a.p, s->st_b.p, s->st_c.p};
+    void *ptrs[] = {s->X, s->V1, s->FdA, s->FdB, s->phase, s->unitsA, s->unitsB, s->stepc,
+                    s->ap_units.p, s->st_a.p, s->st_b.p, s->st_c.p};
     for (void *q : ptrs) if (q) cudaFree(q);
     (void)cudaGetLastError();
     delete s;
@@ -411,18 +386,13 @@ int ds_set_stream(ds_system *s, void *stream) {
     return DS_OK;
 }
 
-int ds_set_tuning(ds_system *s, int32_t j_splits) {
+int ds_set_tuning(ds_system *s, int32_t n_tiles) {
     if (!s) return DS_ERR_NULL;
-    if (j_splits < 0) return DS_ERR_INVALID_PARAM;
+    if (n_tiles < 0) return DS_ERR_INVALID_PARAM;
     DS_TRY(set_device(s));
     CU_TRY(cudaStreamSynchronize(s->stream));
-    s->tune_js = j_splits;
-    const bool f64 = s->P.precision == DS_F64;
-    const int gj = f64 ? group_j<double>() : group_j<float>();
-    const int res = f64 ? ShapeF64::MINB : ShapeF32::MINB;
-    choose_split(s, s->N, s->B, s->n_it, gj, res, &s->JS, &s->jchunk);
-    if (s->partial) { CU_TRY(cudaFree(s->partial)); s->partial = nullptr; }
-    CU_TRY(cudaMalloc((void **)&s->partial, (size_t)s->B * s->JS * 3 * s->Npad * sizeof(double)));
+    s->tune_cta = n_tiles;
+    s->n_cta = choose_tiles(s, s->NQ, s->U, s->B);
     destroy_graphs(s);
     return DS_OK;
 }
@@ -507,13 +477,12 @@ int ds_velocity(ds_system *s, void *V) {
     const bool useB = (s->P.integrator == DS_EULER) && (s->n_host & 1);
     ds::MobArgs A;
     memset(&A, 0, sizeof A);
-    A.N = s->N; A.B = s->B; A.Npad = s->Npad; A.n_it = s->n_it; A.JS = s->JS; A.jchunk = s->jchunk;
-    A.partial = s->partial; A.counters = s->counters;
+    fill_shape(s, A);
     fill_constants(s, A);
     A.mode = ds::EPI_APPLY;
     A.out_u = dV;
-    A.src_pos = useB ? s->pos4B : s->pos4A; A.src_F = useB ? s->F4B : s->F4A; A.Fd_in = useB ? s->FdB : s->FdA;
-    DS_TRY(launch_mob(s, A, false, s->stream));
+    A.src_units = useB ? s->unitsB : s->unitsA; A.Fd_in = useB ? s->FdB : s->FdA;
+    DS_TRY(launch_mob(s, A, s->stream));
     if (!dev) {
         CU_TRY(cudaMemcpyAsync(V, dV, nb, cudaMemcpyDeviceToHost, s->stream));
         CU_TRY(cudaStreamSynchronize(s->stream));
@@ -537,22 +506,25 @@ int ds_mobility_apply(ds_system *s, const void *pos, const void *F, void *u, int
     if (!dF_dev) { DS_TRY(ensure(s->st_b, nb)); CU_TRY(cudaMemcpyAsync(s->st_b.p, F, nb, cudaMemcpyHostToDevice, s->stream)); dF = s->st_b.p; }
     if (!du_dev) { DS_TRY(ensure(s->st_c, nb)); du = s->st_c.p; }
 
-    const int TI = f64 ? tile_i<double>() : tile_i<float>();
-    const int gj = f64 ? group_j<double>() : group_j<float>();
-    const int res = f64 ? ShapeF64::MINB : ShapeF32::MINB;
+    // user arrays -> one beta-stream (pack kernel), then the mobility kernel in EPI_APPLY mode
+    const int U = (n + s->W - 1) / s->W;
+    const long long n_units = (long long)U + ds::PAD_UNITS;
+    DS_TRY(ensure(s->ap_units, (size_t)n_units * ds::UNIT_BYTES));
+    const unsigned pg = (unsigned)((n_units + 255) / 256);
+    if (f64)
+        ds::pack_user_kernel<double><<<pg, 256, 0, s->stream>>>((const double *)dpos, (const double *)dF, (double *)s->ap_units.p, n, n_units);
+    else
+        ds::pack_user_kernel<float><<<pg, 256, 0, s->stream>>>((const float *)dpos, (const float *)dF, (float *)s->ap_units.p, n, n_units);
+    CU_TRY(cudaGetLastError());
+    s->launches += 1;
     ds::MobArgs A;
     memset(&A, 0, sizeof A);
-    A.N = n; A.B = 1; A.n_it = (n + TI - 1) / TI; A.Npad = A.n_it * TI;
-    choose_split(s, n, 1, A.n_it, gj, res, &A.JS, &A.jchunk);
-    if (A.JS > 1) {
-        DS_TRY(ensure(s->ap_partial, (size_t)A.JS * 3 * A.Npad * sizeof(double)));
-        DS_TRY(ensure(s->ap_counters, (size_t)A.n_it * sizeof(unsigned), true));
-    }
-    A.partial = (double *)s->ap_partial.p; A.counters = (unsigned *)s->ap_counters.p;
+    A.N = n; A.B = 1; A.NQ = (n + ds::QI - 1) / ds::QI; A.U = U; A.unit_stride = n_units;
+    A.n_cta = choose_tiles(s, A.NQ, A.U, 1);
     fill_constants(s, A);
     A.mode = ds::EPI_APPLY;
-    A.src_pos = dpos; A.src_F = dF; A.out_u = du;
-    DS_TRY(launch_mob(s, A, true, s->stream));
+    A.src_units = s->ap_units.p; A.out_u = du;
+    DS_TRY(launch_mob(s, A, s->stream));
     if (!du_dev) {
         CU_TRY(cudaMemcpyAsync(u, du, nb, cudaMemcpyDeviceToHost, s->stream));
         CU_TRY(cudaStreamSynchronize(s->stream));

@@ -9,11 +9,12 @@
 namespace ds {
 
 struct StateArgs {
-    int N, B, Npad;
+    int N, B;
+    long long unit_stride;  // units per system in the stream
     const void *user_pos;   // [B][N][3] user precision (init) or NULL
     void *user_out;         // [B][N][3] user precision (forces / get_state)
     double *X;              // [B][N][3]
-    void *pos4, *F4;        // packed T4 [B][Npad]
+    void *units;            // beta-stream T[B][unit_stride][6][W] (mobility.cuh)
     double *Fd;             // [B][N][3]
     const double *phase;    // [B][S]
     long long *counters;    // step counters c[0], c[1]
@@ -34,7 +35,7 @@ __device__ __forceinline__ void dumbbell_force(const double (&x1)[3], const doub
 
 // ds_set_state: X <- user positions; packed copies; forces at t = t0 (step index 0); counters <- 0.
 template <typename T> __global__ void state_init_kernel(const StateArgs A) {
-    typedef typename Pack<T>::T4 T4;
+    constexpr int W = Pack<T>::W;
     const int S = A.N / 2;
     const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (gid == 0) { A.counters[0] = 0; A.counters[1] = 0; }
@@ -51,24 +52,47 @@ template <typename T> __global__ void state_init_kernel(const StateArgs A) {
         A.X[g3 + c] = x1[c]; A.X[g3 + 3 + c] = x2[c];
         A.Fd[g3 + c] = F1[c]; A.Fd[g3 + 3 + c] = -F1[c];
     }
-    T4 *p4 = reinterpret_cast<T4 *>(A.pos4) + (size_t)b * A.Npad + 2 * s;
-    T4 *f4 = reinterpret_cast<T4 *>(A.F4) + (size_t)b * A.Npad + 2 * s;
-    p4[0] = MakeT4<T>::make(x1[0], x1[1], x1[2]);
-    p4[1] = MakeT4<T>::make(x2[0], x2[1], x2[2]);
-    f4[0] = MakeT4<T>::make(F1[0], F1[1], F1[2]);
-    f4[1] = MakeT4<T>::make(-F1[0], -F1[1], -F1[2]);
+    T *un = reinterpret_cast<T *>(A.units) + (size_t)b * A.unit_stride * (6 * W);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        un[unit_index<T>(2LL * s, c)] = (T)x1[c];
+        un[unit_index<T>(2LL * s + 1, c)] = (T)x2[c];
+        un[unit_index<T>(2LL * s, 3 + c)] = (T)F1[c];
+        un[unit_index<T>(2LL * s + 1, 3 + c)] = (T)(-F1[c]);
+    }
 }
 
-// pad entries of the packed arrays: far-away sphere, zero force (never touched afterwards)
-template <typename T> __global__ void pad_init_kernel(void *pos4, void *F4, int N, int Npad, int B) {
-    typedef typename Pack<T>::T4 T4;
-    const int npad = Npad - N;
+// Pad units [U, unit_stride) of every system's stream: far-away spheres with zero force (they
+// contribute exactly 0 to every sum); written once, never touched afterwards.
+template <typename T> __global__ void pad_init_kernel(void *units, int U, long long unit_stride, int B) {
+    constexpr int W = Pack<T>::W;
+    const long long npad = unit_stride - U;
     const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (gid >= (long long)B * npad) return;
-    const int b = (int)(gid / npad), k = (int)(gid % npad);
-    const double far = (double)Pack<T>::dummy();
-    reinterpret_cast<T4 *>(pos4)[(size_t)b * Npad + N + k] = MakeT4<T>::make(far, far, far);
-    reinterpret_cast<T4 *>(F4)[(size_t)b * Npad + N + k] = MakeT4<T>::make(0.0, 0.0, 0.0);
+    const long long b = gid / npad, k = gid % npad;
+    T *un = reinterpret_cast<T *>(units) + ((size_t)b * unit_stride + U + k) * (6 * W);
+#pragma unroll
+    for (int e = 0; e < 6 * W; ++e) un[e] = e < 3 * W ? Pack<T>::dummy() : T(0);
+}
+
+// ds_mobility_apply: user arrays pos, F [n][3] -> one stream of U + PAD_UNITS units (a tail lane of
+// the last unit when n is odd, and all pad units, are far-away zero-force spheres).
+template <typename T> __global__ void pack_user_kernel(const T *__restrict__ pos, const T *__restrict__ F, T *units,
+                                                       int n, long long n_units) {
+    constexpr int W = Pack<T>::W;
+    const long long u = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (u >= n_units) return;
+    T *un = units + (size_t)u * (6 * W);
+#pragma unroll
+    for (int l = 0; l < W; ++l) {
+        const long long i = u * W + l;
+        const bool real = i < n;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            un[c * W + l] = real ? pos[i * 3 + c] : Pack<T>::dummy();
+            un[(3 + c) * W + l] = real ? F[i * 3 + c] : T(0);
+        }
+    }
 }
 
 // ds_forces: Eq. (4) at the current X and t, written in user precision.

@@ -164,8 +164,8 @@ class System:
     def batch_step(self, n_steps):
         _check(lib().ds_batch_step(self._h, int(n_steps)), "ds_batch_step")
 
-    def set_tuning(self, j_splits=0):
-        _check(lib().ds_set_tuning(self._h, int(j_splits)), "ds_set_tuning")
+    def set_tuning(self, n_tiles=0):
+        _check(lib().ds_set_tuning(self._h, int(n_tiles)), "ds_set_tuning")
 
     def launch_count(self):
         return int(lib().ds_launch_count(self._h))

@@ -38,11 +38,11 @@ def dev(x, precision):
     return torch.as_tensor(np.ascontiguousarray(x, dtype=NPDT[precision]), device="cuda")
 
 
-def gpu_apply(X, F, precision, tensor, a=1.0, eta=1.0, j_splits=0, host=False):
+def gpu_apply(X, F, precision, tensor, a=1.0, eta=1.0, n_tiles=0, host=False):
     n = X.shape[0]
     with ds.System(1, precision=precision, tensor=tensor, a=a, eta=eta) as s:
-        if j_splits:
-            s.set_tuning(j_splits)
+        if n_tiles:
+            s.set_tuning(n_tiles)
         if host:
             Xh = np.ascontiguousarray(X, dtype=NPDT[precision])
             Fh = np.ascontiguousarray(F, dtype=NPDT[precision])
@@ -90,11 +90,12 @@ def test_apply_parity_config4_full_size(tensor, precision):
 
 
 @pytest.mark.parametrize("precision", [ds.F32, ds.F64])
-@pytest.mark.parametrize("j_splits", [1, 2, 5, 16])
-def test_apply_parity_forced_splits(j_splits, precision):
-    """The split-j partial-sum path and the single-block path give the same answer."""
+@pytest.mark.parametrize("n_tiles", [1, 2, 5, 16, 100, 384])
+def test_apply_parity_forced_tiles(n_tiles, precision):
+    """Every (alpha-thread, beta-group) shape of the CTA gives the same answer: 1 tile = 384 quads x 1
+    beta-group ... 384 tiles = 1 quad x 512 beta-groups."""
     X, F = inputs.apply_case(1536, 21, 22)
-    u = gpu_apply(X, F, precision, ds.RPY, j_splits=j_splits)
+    u = gpu_apply(X, F, precision, ds.RPY, n_tiles=n_tiles)
     assert rel_l2(u, oracle_apply(X, F, precision, ds.RPY)) <= TOL[precision]
 
 
