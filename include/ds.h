@@ -111,9 +111,10 @@ int ds_mobility_apply(ds_system *s, const void *pos, const void *F, void *u, int
 
 /* Advance the state by n_steps explicit steps: Heun = predictor X* = X + dt V(X,t_n),
  * corrector X <- X + dt/2 (V(X,t_n) + V(X*,t_n + dt)); Euler = X <- X + dt V(X,t_n);
- * V(X,t) = H(X) F(X,t).  The whole loop runs on the device (CUDA graph replays, no host round
- * trip per step).  ds_step requires n_batch == 1 (DS_ERR_STATE otherwise); ds_batch_step advances
- * all B systems by n_steps each.  n_steps >= 0.                                                 */
+ * V(X,t) = H(X) F(X,t).  The whole loop runs on the device: one persistent kernel launch per
+ * call (per 65536 steps) and per group of co-resident systems, no host round trip per step.
+ * ds_step requires n_batch == 1 (DS_ERR_STATE otherwise); ds_batch_step advances all B systems
+ * by n_steps each.  n_steps >= 0.                                                               */
 int ds_step(ds_system *s, int64_t n_steps);
 int ds_batch_step(ds_system *s, int64_t n_steps);
 
@@ -122,8 +123,13 @@ int ds_batch_step(ds_system *s, int64_t n_steps);
 int ds_velocity(ds_system *s, void *V);
 
 /* Launch-shape override for tuning and tests: number of row tiles (CTAs) per system; 0 = library
- * heuristic.  Values below ceil(ceil(N/4)/512) or above ceil(N/4) are clamped.                   */
+ * heuristic.  Values below ceil(ceil(N/4)/512) or above ceil(N/4) are clamped; the step modes also
+ * clamp to the SM count (their CTAs meet at a barrier every stage and must be co-resident).      */
 int ds_set_tuning(ds_system *s, int32_t n_tiles);
+
+/* Development instrumentation: device_buffer (DEVICE pointer, 16 int64 per CTA of the largest launch,
+ * or NULL to switch off) receives clock64() samples of the last stage of every hot-kernel launch.  */
+int ds_set_probe(ds_system *s, void *device_buffer);
 
 /* Number of kernels launched by this system since creation (bench.py's gpu_launches claim). */
 int64_t ds_launch_count(const ds_system *s);

@@ -48,32 +48,36 @@ struct Buf {
 struct ds_system {
     ds_params P;
     cudaStream_t stream = nullptr;
-    cudaStream_t cap_stream = nullptr;
     int num_sms = 148;
     int N = 0, B = 0, S = 0;
     int W = 1;                  // spheres per unit: 2 (FP32 packs) or 1 (FP64)
     int NQ = 0, U = 0;          // quads = ceil(N/4), units = ceil(N/W)
     long long unit_stride = 0;  // units per system in the streams
-    int tune_cta = 0, n_cta = 1;
+    int tune_cta = 0;
+    // launch shape of the step modes (ds_step, ds_batch_step, ds_velocity)
+    int n_cta = 1;              // row tiles (CTAs) per system
+    int sys_per_launch = 1;     // systems advanced by one launch (co-residency: n_cta * sys_per_launch <= SMs)
+    int ns = ds::NS_MAX;        // ring slots
+    int state_smem = 1;         // per-row state in shared memory (else in the global arrays below)
+    size_t smem_bytes = 0;
     bool has_state = false;
     double t0 = 0.0;
-    long long n_host = 0;  // mirror of the device step counter
+    long long n_host = 0;       // steps taken since ds_set_state
     int64_t launches = 0;
     // state
-    double *X = nullptr, *V1 = nullptr, *FdA = nullptr, *FdB = nullptr, *phase = nullptr;
-    void *unitsA = nullptr, *unitsB = nullptr;  // beta-streams (mobility.cuh), ping-pong
-    long long *stepc = nullptr;                 // c[0], c[1]
-    // graphs
-    cudaGraphExec_t graphK = nullptr;  // GRAPH_STEPS steps
-    int graph_steps = 0;
-    int graph_nodes = 0;
+    double *X = nullptr, *phase = nullptr;
+    void *units[2] = {nullptr, nullptr};        // beta-streams (mobility.cuh), ping-pong over the stages
+    unsigned long long *bar = nullptr;          // [B] arrival counters of the inter-CTA barrier
+    unsigned long long bar_base = 0;
+    double *Xcg = nullptr, *V1g = nullptr, *Fg = nullptr, *Lg = nullptr;  // only when !state_smem
+    long long *probe = nullptr;                 // caller's device buffer (ds_set_probe) or NULL
     // scratch of the stateless apply and of host-pointer staging
     Buf ap_units, st_a, st_b, st_c;
 };
 
 namespace {
 
-constexpr int GRAPH_STEPS = 32;
+constexpr long long MAX_STEPS_PER_LAUNCH = 1LL << 16;
 
 int ensure(Buf &b, size_t bytes, bool zero = false) {
     if (b.cap >= bytes) return DS_OK;
@@ -101,10 +105,10 @@ int is_device_ptr(const void *p, int *out) {
 
 size_t elem_size(const ds_system *s) { return s->P.precision == DS_F64 ? sizeof(double) : sizeof(float); }
 
-// Launch shape: n_cta row tiles per system (mobility.cuh).  Every CTA walks all U units with
-// n_jg = NT / nq beta-groups, i.e. ceil(U / n_jg) iterations of 4 alpha x 1 unit per thread, so the
-// modelled time of a launch is waves x (iterations + a fixed per-CTA cost, in iterations).
-int choose_tiles(const ds_system *s, int NQ, int U, int B) {
+// Launch shape of the stateless apply: n_cta row tiles (mobility.cuh), any number of waves.  Every CTA
+// walks all U units with n_jg = NT / nq beta-groups, i.e. ceil(U / n_jg) iterations of 4 alpha x 1 unit
+// per thread, so the modelled time is waves x (iterations + a fixed per-CTA cost, in iterations).
+int choose_tiles_apply(const ds_system *s, int NQ, int U) {
     const int lo = (NQ + ds::NT - 1) / ds::NT;  // nq <= NT
     if (s->tune_cta > 0) {
         int t = s->tune_cta < lo ? lo : s->tune_cta;
@@ -117,38 +121,84 @@ int choose_tiles(const ds_system *s, int NQ, int U, int B) {
         const int nq = (NQ + n - 1) / n;
         const int n_jg = ds::NT / nq;
         const long long iters = (U + n_jg - 1) / n_jg;
-        const long long waves = ((long long)B * n + s->num_sms - 1) / s->num_sms;
+        const long long waves = ((long long)n + s->num_sms - 1) / s->num_sms;
         const double cost = (double)waves * ((double)iters + 6.0);
         if (cost < best_cost * (1.0 - 1e-9)) { best_cost = cost; best = n; }
     }
     return best;
 }
 
-template <typename T, int TENSOR> int launch_mob_t(ds_system *s, const ds::MobArgs &A, cudaStream_t st) {
-    auto kern = ds::mobility_kernel<T, TENSOR>;
+// Launch shape of the step modes: all CTAs of a launch are co-resident (they meet at the inter-CTA
+// barrier every stage), so n_cta <= SMs and floor(SMs / n_cta) systems run per launch; B systems take
+// ceil(B / that) launches one after the other.  Same cost model, plus the barrier in the fixed cost.
+int choose_shape_step(ds_system *s) {
+    const int lo = (s->NQ + ds::NT - 1) / ds::NT;
+    if (lo > s->num_sms) return DS_ERR_INVALID_PARAM;
+    int hi = s->NQ < s->num_sms ? s->NQ : s->num_sms;
+    int best = lo;
+    if (s->tune_cta > 0) {
+        best = s->tune_cta < lo ? lo : (s->tune_cta > hi ? hi : s->tune_cta);
+    } else {
+        double best_cost = 1e300;
+        for (int n = lo; n <= hi; ++n) {
+            const int nq = (s->NQ + n - 1) / n;
+            const int n_jg = ds::NT / nq;
+            const long long iters = (s->U + n_jg - 1) / n_jg;
+            int per = s->num_sms / n;
+            per = per < 1 ? 1 : (per > s->B ? s->B : per);
+            const long long groups = (s->B + per - 1) / per;
+            const double cost = (double)groups * ((double)iters + (n > 1 ? 5.0 : 3.0));
+            if (cost < best_cost * (1.0 - 1e-9)) { best_cost = cost; best = n; }
+        }
+    }
+    s->n_cta = best;
+    int per = best > 1 ? s->num_sms / best : s->B;   // n_cta == 1: systems never wait on one another
+    s->sys_per_launch = per < 1 ? 1 : (per > s->B ? s->B : per);
+    const int rows_max = 4 * ((s->NQ + best - 1) / best);
+    const size_t state = (size_t)rows_max * ds::STATE_BYTES_PER_ROW;
+    const long long room = (long long)ds::SMEM_MAX - ds::BAR_BYTES - (long long)state;
+    if (room >= (long long)ds::NS_MIN * ds::SLOT_BYTES) {
+        s->state_smem = 1;
+        s->ns = (int)(room / ds::SLOT_BYTES);
+        if (s->ns > ds::NS_MAX) s->ns = ds::NS_MAX;
+        s->smem_bytes = (size_t)s->ns * ds::SLOT_BYTES + ds::BAR_BYTES + state;
+    } else {
+        s->state_smem = 0;
+        s->ns = ds::NS_MAX;
+        s->smem_bytes = (size_t)s->ns * ds::SLOT_BYTES + ds::BAR_BYTES;
+    }
+    return DS_OK;
+}
+
+template <typename T, int TENSOR>
+int launch_run_t(ds_system *s, ds::RunArgs &A, dim3 grid, size_t smem, bool coop, cudaStream_t st) {
+    auto kern = ds::run_kernel<T, TENSOR>;
     static bool attr_done = false;
     if (!attr_done) {
-        CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, ds::SMEM_BYTES));
+        CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, ds::SMEM_MAX));
         attr_done = true;
     }
-    dim3 grid((unsigned)A.n_cta, (unsigned)A.B), block(ds::NT);
-    kern<<<grid, block, ds::SMEM_BYTES, st>>>(A);
-    CU_TRY(cudaGetLastError());
+    if (coop) {
+        void *args[] = {(void *)&A};
+        CU_TRY(cudaLaunchCooperativeKernel((const void *)kern, grid, dim3(ds::NT), args, smem, st));
+    } else {
+        kern<<<grid, dim3(ds::NT), smem, st>>>(A);
+        CU_TRY(cudaGetLastError());
+    }
     s->launches += 1;
     return DS_OK;
 }
 
-int launch_mob(ds_system *s, const ds::MobArgs &A, cudaStream_t st) {
+int launch_run(ds_system *s, ds::RunArgs &A, dim3 grid, size_t smem, bool coop, cudaStream_t st) {
     const bool f64 = s->P.precision == DS_F64, rpy = s->P.tensor == DS_RPY;
-    if (f64) return rpy ? launch_mob_t<double, ds::TENSOR_RPY>(s, A, st) : launch_mob_t<double, ds::TENSOR_OSEEN>(s, A, st);
-    return rpy ? launch_mob_t<float, ds::TENSOR_RPY>(s, A, st) : launch_mob_t<float, ds::TENSOR_OSEEN>(s, A, st);
+    if (f64)
+        return rpy ? launch_run_t<double, ds::TENSOR_RPY>(s, A, grid, smem, coop, st)
+                   : launch_run_t<double, ds::TENSOR_OSEEN>(s, A, grid, smem, coop, st);
+    return rpy ? launch_run_t<float, ds::TENSOR_RPY>(s, A, grid, smem, coop, st)
+               : launch_run_t<float, ds::TENSOR_OSEEN>(s, A, grid, smem, coop, st);
 }
 
-void fill_shape(const ds_system *s, ds::MobArgs &A) {
-    A.N = s->N; A.B = s->B; A.NQ = s->NQ; A.U = s->U; A.n_cta = s->n_cta; A.unit_stride = s->unit_stride;
-}
-
-void fill_constants(const ds_system *s, ds::MobArgs &A) {
+void fill_constants(const ds_system *s, ds::RunArgs &A) {
     const double pi = 3.14159265358979323846264338327950288;
     A.self_mob = 1.0 / (6.0 * pi * s->P.eta * s->P.a);
     A.pre = 1.0 / (8.0 * pi * s->P.eta);
@@ -157,67 +207,27 @@ void fill_constants(const ds_system *s, ds::MobArgs &A) {
     A.t0 = s->t0; A.dt = s->P.dt; A.ell = s->P.ell; A.lambda = s->P.lambda; A.omega = s->P.omega; A.k0 = s->P.k0;
 }
 
-// One stage of the integrator on the system's own state.  set 0: (unitsA,FdA) -> writes set B
-// (predictor) ; set 1: reads B, writes A (corrector).  Euler reads A and writes A... see below.
-int launch_state_stage(ds_system *s, int mode, int cr, int cw, long long inc, cudaStream_t st) {
-    ds::MobArgs A;
+// RUN_VELOCITY (n_steps ignored) or RUN_STEP on the system's own state: one launch per group of
+// co-resident systems; the barrier counters advance by n_cta per stage.
+int launch_state_run(ds_system *s, int mode, long long n_steps, void *out_u) {
+    ds::RunArgs A;
     memset(&A, 0, sizeof A);
-    fill_shape(s, A);
+    A.N = s->N; A.NQ = s->NQ; A.U = s->U; A.n_cta = s->n_cta; A.ns = s->ns; A.unit_stride = s->unit_stride;
+    A.units[0] = s->units[0]; A.units[1] = s->units[1]; A.cur = 0;
     fill_constants(s, A);
-    A.mode = mode;
-    A.X = s->X; A.V1 = s->V1; A.phase = s->phase;
-    A.n_read = s->stepc + cr; A.n_write = s->stepc + cw; A.n_inc = inc;
-    const bool fromB = (mode == ds::EPI_CORR);
-    A.src_units = fromB ? s->unitsB : s->unitsA;
-    A.Fd_in = fromB ? s->FdB : s->FdA;
-    const bool toB = (mode == ds::EPI_PRED);
-    A.units_out = toB ? s->unitsB : s->unitsA;
-    A.Fd_out = toB ? s->FdB : s->FdA;
-    return launch_mob(s, A, st);
-}
-
-// One full step.  Heun: PRED (reads c[0], writes c[1] = n) then CORR (reads c[1], writes c[0] = n+1).
-// Euler: in place on set A is NOT safe (other blocks still read unitsA), so Euler ping-pongs the
-// packed sets: even steps read A write B, odd steps read B write A; the counters ping-pong too.
-int launch_one_step(ds_system *s, long long n_index, cudaStream_t st) {
-    if (s->P.integrator == DS_HEUN) {
-        DS_TRY(launch_state_stage(s, ds::EPI_PRED, 0, 1, 0, st));
-        return launch_state_stage(s, ds::EPI_CORR, 1, 0, 1, st);
+    A.mode = mode; A.heun = s->P.integrator == DS_HEUN ? 1 : 0;
+    A.n0 = s->n_host; A.n_steps = n_steps; A.out_u = out_u;
+    A.X = s->X; A.phase = s->phase;
+    A.bar = s->bar; A.bar_base = s->bar_base;
+    A.state_smem = s->state_smem; A.Xcg = s->Xcg; A.V1g = s->V1g; A.Fg = s->Fg; A.Lg = s->Lg;
+    A.probe = s->probe;
+    const long long n_stage = mode == ds::RUN_STEP ? n_steps * (A.heun ? 2 : 1) : 1;
+    for (int b0 = 0; b0 < s->B; b0 += s->sys_per_launch) {
+        const int nb = s->B - b0 < s->sys_per_launch ? s->B - b0 : s->sys_per_launch;
+        A.b0 = b0;
+        DS_TRY(launch_run(s, A, dim3((unsigned)s->n_cta, (unsigned)nb), s->smem_bytes, s->n_cta > 1, s->stream));
     }
-    const int par = (int)(n_index & 1);
-    ds::MobArgs A;
-    memset(&A, 0, sizeof A);
-    fill_shape(s, A);
-    fill_constants(s, A);
-    A.mode = ds::EPI_EULER;
-    A.X = s->X; A.V1 = s->V1; A.phase = s->phase;
-    A.n_read = s->stepc + par; A.n_write = s->stepc + (par ^ 1); A.n_inc = 1;
-    A.src_units = par ? s->unitsB : s->unitsA; A.Fd_in = par ? s->FdB : s->FdA;
-    A.units_out = par ? s->unitsA : s->unitsB; A.Fd_out = par ? s->FdA : s->FdB;
-    return launch_mob(s, A, st);
-}
-
-void destroy_graphs(ds_system *s) {
-    if (s->graphK) { cudaGraphExecDestroy(s->graphK); s->graphK = nullptr; }
-    s->graph_steps = 0;
-}
-
-int build_graph(ds_system *s) {
-    destroy_graphs(s);
-    cudaGraph_t g = nullptr;
-    const int64_t before = s->launches;
-    CU_TRY(cudaStreamBeginCapture(s->cap_stream, cudaStreamCaptureModeThreadLocal));
-    int rc = DS_OK;
-    for (int k = 0; k < GRAPH_STEPS && rc == DS_OK; ++k) rc = launch_one_step(s, k, s->cap_stream);  // parity 0 start
-    cudaError_t e = cudaStreamEndCapture(s->cap_stream, &g);
-    s->graph_nodes = (int)(s->launches - before);
-    s->launches = before;
-    if (rc != DS_OK) { if (g) cudaGraphDestroy(g); return rc; }
-    CU_TRY(e);
-    e = cudaGraphInstantiate(&s->graphK, g, 0);
-    cudaGraphDestroy(g);
-    CU_TRY(e);
-    s->graph_steps = GRAPH_STEPS;
+    if (s->n_cta > 1) s->bar_base += (unsigned long long)s->n_cta * (unsigned long long)n_stage;
     return DS_OK;
 }
 
@@ -229,11 +239,9 @@ int set_device(const ds_system *s) {
 template <typename T> int run_state_init(ds_system *s, const void *dpos) {
     ds::StateArgs A;
     memset(&A, 0, sizeof A);
-    A.N = s->N; A.B = s->B; A.unit_stride = s->unit_stride; A.user_pos = dpos; A.X = s->X; A.units = s->unitsA;
-    A.Fd = s->FdA; A.phase = s->phase; A.counters = s->stepc; A.t = s->t0;
-    A.ell = s->P.ell; A.lambda = s->P.lambda; A.omega = s->P.omega; A.k0 = s->P.k0;
-    const long long n = (long long)s->B * s->S;
-    ds::state_init_kernel<T><<<(unsigned)((n + 127) / 128), 128, 0, s->stream>>>(A);
+    A.N = s->N; A.B = s->B; A.user_pos = dpos; A.X = s->X;
+    const long long n = (long long)s->B * s->N * 3;
+    ds::state_init_kernel<T><<<(unsigned)((n + 255) / 256), 256, 0, s->stream>>>(A);
     CU_TRY(cudaGetLastError());
     s->launches += 1;
     return DS_OK;
@@ -242,7 +250,7 @@ template <typename T> int run_state_init(ds_system *s, const void *dpos) {
 template <typename T> int run_forces_out(ds_system *s, void *dF) {
     ds::StateArgs A;
     memset(&A, 0, sizeof A);
-    A.N = s->N; A.B = s->B; A.unit_stride = s->unit_stride; A.user_out = dF; A.X = s->X; A.phase = s->phase;
+    A.N = s->N; A.B = s->B; A.user_out = dF; A.X = s->X; A.phase = s->phase;
     A.t = s->t0 + (double)s->n_host * s->P.dt;
     A.ell = s->P.ell; A.lambda = s->P.lambda; A.omega = s->P.omega; A.k0 = s->P.k0;
     const long long n = (long long)s->B * s->S;
@@ -345,21 +353,22 @@ int ds_create(const ds_params *p, ds_system **out) {
     int rc = DS_OK;
     auto fail = [&](int code) { ds_destroy(s); return code; };
     if (set_device(s) != DS_OK) return fail(DS_ERR_CUDA);
-    if (cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking) != cudaSuccess) return fail(DS_ERR_CUDA);
+    rc = choose_shape_step(s);   // N too large for one co-resident grid: the step modes cannot run
+    if (rc != DS_OK) return fail(rc);
     const size_t n3 = (size_t)s->B * s->N * 3;
     const size_t ub = (size_t)s->B * (size_t)s->unit_stride * ds::UNIT_BYTES;
     cudaError_t e = cudaSuccess;
     auto al = [&](void **ptr, size_t bytes) { if (e == cudaSuccess) e = cudaMalloc(ptr, bytes); };
-    al((void **)&s->X, n3 * 8); al((void **)&s->V1, n3 * 8); al((void **)&s->FdA, n3 * 8); al((void **)&s->FdB, n3 * 8);
+    al((void **)&s->X, n3 * 8);
     al((void **)&s->phase, (size_t)s->B * s->S * 8);
-    al(&s->unitsA, ub); al(&s->unitsB, ub);
-    al((void **)&s->stepc, 2 * sizeof(long long));
+    al(&s->units[0], ub); al(&s->units[1], ub);
+    al((void **)&s->bar, (size_t)s->B * sizeof(unsigned long long));
+    // global homes of the per-row state, used only by tiles too large for shared memory (any tuning)
+    al((void **)&s->Xcg, n3 * 8); al((void **)&s->V1g, n3 * 8); al((void **)&s->Fg, n3 * 8);
+    al((void **)&s->Lg, (size_t)s->B * s->S * 8);
     if (e != cudaSuccess) { snprintf(g_cuda_err, sizeof g_cuda_err, "cudaMalloc -> %s", cudaGetErrorString(e)); (void)cudaGetLastError(); return fail(DS_ERR_ALLOC); }
-    if (cudaMemset(s->stepc, 0, 2 * sizeof(long long)) != cudaSuccess) return fail(DS_ERR_CUDA);
-    rc = f64 ? run_pad_init<double>(s, s->unitsA) : run_pad_init<float>(s, s->unitsA);
-    if (rc == DS_OK) rc = f64 ? run_pad_init<double>(s, s->unitsB) : run_pad_init<float>(s, s->unitsB);
-    if (rc != DS_OK) return fail(rc);
-    rc = ds_set_tuning(s, 0);
+    if (cudaMemsetAsync(s->bar, 0, (size_t)s->B * sizeof(unsigned long long), s->stream) != cudaSuccess) return fail(DS_ERR_CUDA);
+    for (int k = 0; k < 2 && rc == DS_OK; ++k) rc = f64 ? run_pad_init<double>(s, s->units[k]) : run_pad_init<float>(s, s->units[k]);
     if (rc != DS_OK) return fail(rc);
     if (cudaStreamSynchronize(s->stream) != cudaSuccess) return fail(DS_ERR_CUDA);
     *out = s;
@@ -370,9 +379,7 @@ int ds_destroy(ds_system *s) {
     if (!s) return DS_OK;
     cudaSetDevice(s->P.device);
     cudaStreamSynchronize(s->stream);
-    destroy_graphs(s);
-    if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
-    void *ptrs[] = {s->X, s->V1, s->FdA, s->FdB, s->phase, s->unitsA, s->unitsB, s->stepc,
+    void *ptrs[] = {s->X, s->phase, s->units[0], s->units[1], s->bar, s->Xcg, s->V1g, s->Fg, s->Lg,
                     s->ap_units.p, s->st_a.p, s->st_b.p, s->st_c.p};
     for (void *q : ptrs) if (q) cudaFree(q);
     (void)cudaGetLastError();
@@ -392,8 +399,12 @@ int ds_set_tuning(ds_system *s, int32_t n_tiles) {
     DS_TRY(set_device(s));
     CU_TRY(cudaStreamSynchronize(s->stream));
     s->tune_cta = n_tiles;
-    s->n_cta = choose_tiles(s, s->NQ, s->U, s->B);
-    destroy_graphs(s);
+    return choose_shape_step(s);
+}
+
+int ds_set_probe(ds_system *s, void *device_buffer) {
+    if (!s) return DS_ERR_NULL;
+    s->probe = (long long *)device_buffer;
     return DS_OK;
 }
 
@@ -416,7 +427,6 @@ int ds_set_state(ds_system *s, const void *pos, const void *phase, double t0) {
     }
     s->t0 = t0;
     s->n_host = 0;
-    if (s->graphK) destroy_graphs(s);  // t0 is baked into the graph's kernel arguments
     DS_TRY(s->P.precision == DS_F64 ? run_state_init<double>(s, dpos) : run_state_init<float>(s, dpos));
     s->has_state = true;
     return DS_OK;
@@ -473,16 +483,7 @@ int ds_velocity(ds_system *s, void *V) {
     DS_TRY(is_device_ptr(V, &dev));
     void *dV = V;
     if (!dev) { DS_TRY(ensure(s->st_c, nb)); dV = s->st_c.p; }
-    // the packed set that holds the current state: A for Heun; for Euler it ping-pongs with the step parity
-    const bool useB = (s->P.integrator == DS_EULER) && (s->n_host & 1);
-    ds::MobArgs A;
-    memset(&A, 0, sizeof A);
-    fill_shape(s, A);
-    fill_constants(s, A);
-    A.mode = ds::EPI_APPLY;
-    A.out_u = dV;
-    A.src_units = useB ? s->unitsB : s->unitsA; A.Fd_in = useB ? s->FdB : s->FdA;
-    DS_TRY(launch_mob(s, A, s->stream));
+    DS_TRY(launch_state_run(s, ds::RUN_VELOCITY, 0, dV));
     if (!dev) {
         CU_TRY(cudaMemcpyAsync(V, dV, nb, cudaMemcpyDeviceToHost, s->stream));
         CU_TRY(cudaStreamSynchronize(s->stream));
@@ -506,7 +507,7 @@ int ds_mobility_apply(ds_system *s, const void *pos, const void *F, void *u, int
     if (!dF_dev) { DS_TRY(ensure(s->st_b, nb)); CU_TRY(cudaMemcpyAsync(s->st_b.p, F, nb, cudaMemcpyHostToDevice, s->stream)); dF = s->st_b.p; }
     if (!du_dev) { DS_TRY(ensure(s->st_c, nb)); du = s->st_c.p; }
 
-    // user arrays -> one beta-stream (pack kernel), then the mobility kernel in EPI_APPLY mode
+    // user arrays -> one beta-stream (pack kernel), then the mobility kernel in RUN_APPLY mode
     const int U = (n + s->W - 1) / s->W;
     const long long n_units = (long long)U + ds::PAD_UNITS;
     DS_TRY(ensure(s->ap_units, (size_t)n_units * ds::UNIT_BYTES));
@@ -517,14 +518,16 @@ int ds_mobility_apply(ds_system *s, const void *pos, const void *F, void *u, int
         ds::pack_user_kernel<float><<<pg, 256, 0, s->stream>>>((const float *)dpos, (const float *)dF, (float *)s->ap_units.p, n, n_units);
     CU_TRY(cudaGetLastError());
     s->launches += 1;
-    ds::MobArgs A;
+    ds::RunArgs A;
     memset(&A, 0, sizeof A);
-    A.N = n; A.B = 1; A.NQ = (n + ds::QI - 1) / ds::QI; A.U = U; A.unit_stride = n_units;
-    A.n_cta = choose_tiles(s, A.NQ, A.U, 1);
+    A.N = n; A.NQ = (n + ds::QI - 1) / ds::QI; A.U = U; A.unit_stride = n_units;
+    A.n_cta = choose_tiles_apply(s, A.NQ, A.U);
+    A.ns = ds::NS_MAX;
     fill_constants(s, A);
-    A.mode = ds::EPI_APPLY;
-    A.src_units = s->ap_units.p; A.out_u = du;
-    DS_TRY(launch_mob(s, A, s->stream));
+    A.mode = ds::RUN_APPLY;
+    A.units[0] = s->ap_units.p; A.units[1] = s->ap_units.p; A.out_u = du;
+    A.probe = s->probe;
+    DS_TRY(launch_run(s, A, dim3((unsigned)A.n_cta, 1), (size_t)ds::NS_MAX * ds::SLOT_BYTES + ds::BAR_BYTES, false, s->stream));
     if (!du_dev) {
         CU_TRY(cudaMemcpyAsync(u, du, nb, cudaMemcpyDeviceToHost, s->stream));
         CU_TRY(cudaStreamSynchronize(s->stream));
@@ -538,22 +541,10 @@ int ds_batch_step(ds_system *s, int64_t n_steps) {
     if (!s->has_state) return DS_ERR_STATE;
     DS_TRY(set_device(s));
     int64_t left = n_steps;
-    // graphs start at even step parity (Euler ping-pong); GRAPH_STEPS is even
-    while (left > 0 && ((s->n_host & 1) != 0 || left < GRAPH_STEPS)) {
-        DS_TRY(launch_one_step(s, s->n_host, s->stream));
-        s->n_host += 1; left -= 1;
-    }
-    if (left >= GRAPH_STEPS) {
-        if (!s->graphK) DS_TRY(build_graph(s));
-        while (left >= GRAPH_STEPS) {
-            CU_TRY(cudaGraphLaunch(s->graphK, s->stream));
-            s->launches += s->graph_nodes;
-            s->n_host += GRAPH_STEPS; left -= GRAPH_STEPS;
-        }
-    }
-    while (left > 0) {
-        DS_TRY(launch_one_step(s, s->n_host, s->stream));
-        s->n_host += 1; left -= 1;
+    while (left > 0) {   // one launch runs up to MAX_STEPS_PER_LAUNCH steps entirely on the device
+        const long long k = left < MAX_STEPS_PER_LAUNCH ? left : MAX_STEPS_PER_LAUNCH;
+        DS_TRY(launch_state_run(s, ds::RUN_STEP, k, nullptr));
+        s->n_host += k; left -= k;
     }
     return DS_OK;
 }

@@ -22,7 +22,7 @@ ERR_INVALID_PARAM, ERR_NULL, ERR_CUDA, ERR_STATE, ERR_NO_DEVICE, ERR_ALLOC = -1,
 
 # every symbol include/ds.h declares (tests check that the built library exports all of them)
 SYMBOLS = ["ds_create", "ds_destroy", "ds_set_stream", "ds_set_state", "ds_get_state", "ds_forces",
-           "ds_mobility_apply", "ds_step", "ds_batch_step", "ds_velocity", "ds_set_tuning", "ds_launch_count",
+           "ds_mobility_apply", "ds_step", "ds_batch_step", "ds_velocity", "ds_set_tuning", "ds_set_probe", "ds_launch_count",
            "ds_peak_probe", "ds_strerror", "ds_last_cuda_error", "ds_version"]
 
 
@@ -65,6 +65,7 @@ def lib():
         L.ds_batch_step.argtypes = [vp, i64]
         L.ds_velocity.argtypes = [vp, vp]
         L.ds_set_tuning.argtypes = [vp, i32]
+        L.ds_set_probe.argtypes = [vp, vp]
         L.ds_launch_count.argtypes = [vp]
         L.ds_launch_count.restype = i64
         L.ds_peak_probe.argtypes = [i32, i32, ctypes.POINTER(dbl)]
@@ -166,6 +167,9 @@ class System:
 
     def set_tuning(self, n_tiles=0):
         _check(lib().ds_set_tuning(self._h, int(n_tiles)), "ds_set_tuning")
+
+    def set_probe(self, buf=None):
+        _check(lib().ds_set_probe(self._h, _ptr(buf)), "ds_set_probe")
 
     def launch_count(self):
         return int(lib().ds_launch_count(self._h))
