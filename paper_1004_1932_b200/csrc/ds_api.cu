@@ -57,7 +57,7 @@ struct ds_system {
     // launch shape of the step modes (ds_step, ds_batch_step, ds_velocity)
     int n_cta = 1;              // row tiles (CTAs) per system
     int sys_per_launch = 1;     // systems advanced by one launch (co-residency: n_cta * sys_per_launch <= SMs)
-    int ns = ds::NS_MAX;        // ring slots
+    int buf_bytes = 0;          // shared-memory stream buffer of the step modes
     int state_smem = 1;         // per-row state in shared memory (else in the global arrays below)
     size_t smem_bytes = 0;
     bool has_state = false;
@@ -156,16 +156,15 @@ int choose_shape_step(ds_system *s) {
     s->sys_per_launch = per < 1 ? 1 : (per > s->B ? s->B : per);
     const int rows_max = 4 * ((s->NQ + best - 1) / best);
     const size_t state = (size_t)rows_max * ds::STATE_BYTES_PER_ROW;
-    const long long room = (long long)ds::SMEM_MAX - ds::BAR_BYTES - (long long)state;
+    const long long room = ((long long)ds::SMEM_MAX - ds::BAR_BYTES - (long long)state) / 128 * 128;
     if (room >= (long long)ds::NS_MIN * ds::SLOT_BYTES) {
         s->state_smem = 1;
-        s->ns = (int)(room / ds::SLOT_BYTES);
-        if (s->ns > ds::NS_MAX) s->ns = ds::NS_MAX;
-        s->smem_bytes = (size_t)s->ns * ds::SLOT_BYTES + ds::BAR_BYTES + state;
+        s->buf_bytes = (int)room;
+        s->smem_bytes = (size_t)room + ds::BAR_BYTES + state;
     } else {
         s->state_smem = 0;
-        s->ns = ds::NS_MAX;
-        s->smem_bytes = (size_t)s->ns * ds::SLOT_BYTES + ds::BAR_BYTES;
+        s->buf_bytes = (ds::SMEM_MAX - ds::BAR_BYTES) / 128 * 128;
+        s->smem_bytes = (size_t)s->buf_bytes + ds::BAR_BYTES;
     }
     return DS_OK;
 }
@@ -204,6 +203,7 @@ void fill_constants(const ds_system *s, ds::RunArgs &A) {
     A.pre = 1.0 / (8.0 * pi * s->P.eta);
     A.c1 = 2.0 * s->P.a * s->P.a / 3.0;
     A.c2 = 2.0 * s->P.a * s->P.a;
+    A.c1f = (float)A.c1; A.c2f = (float)A.c2;
     A.t0 = s->t0; A.dt = s->P.dt; A.ell = s->P.ell; A.lambda = s->P.lambda; A.omega = s->P.omega; A.k0 = s->P.k0;
 }
 
@@ -212,7 +212,7 @@ void fill_constants(const ds_system *s, ds::RunArgs &A) {
 int launch_state_run(ds_system *s, int mode, long long n_steps, void *out_u) {
     ds::RunArgs A;
     memset(&A, 0, sizeof A);
-    A.N = s->N; A.NQ = s->NQ; A.U = s->U; A.n_cta = s->n_cta; A.ns = s->ns; A.unit_stride = s->unit_stride;
+    A.N = s->N; A.NQ = s->NQ; A.U = s->U; A.n_cta = s->n_cta; A.buf_bytes = s->buf_bytes; A.unit_stride = s->unit_stride;
     A.units[0] = s->units[0]; A.units[1] = s->units[1]; A.cur = 0;
     fill_constants(s, A);
     A.mode = mode; A.heun = s->P.integrator == DS_HEUN ? 1 : 0;
@@ -522,12 +522,12 @@ int ds_mobility_apply(ds_system *s, const void *pos, const void *F, void *u, int
     memset(&A, 0, sizeof A);
     A.N = n; A.NQ = (n + ds::QI - 1) / ds::QI; A.U = U; A.unit_stride = n_units;
     A.n_cta = choose_tiles_apply(s, A.NQ, A.U);
-    A.ns = ds::NS_MAX;
+    A.buf_bytes = (ds::SMEM_MAX - ds::BAR_BYTES) / 128 * 128;
     fill_constants(s, A);
     A.mode = ds::RUN_APPLY;
     A.units[0] = s->ap_units.p; A.units[1] = s->ap_units.p; A.out_u = du;
     A.probe = s->probe;
-    DS_TRY(launch_run(s, A, dim3((unsigned)A.n_cta, 1), (size_t)ds::NS_MAX * ds::SLOT_BYTES + ds::BAR_BYTES, false, s->stream));
+    DS_TRY(launch_run(s, A, dim3((unsigned)A.n_cta, 1), (size_t)A.buf_bytes + ds::BAR_BYTES, false, s->stream));
     if (!du_dev) {
         CU_TRY(cudaMemcpyAsync(u, du, nb, cudaMemcpyDeviceToHost, s->stream));
         CU_TRY(cudaStreamSynchronize(s->stream));

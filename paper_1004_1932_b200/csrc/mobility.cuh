@@ -49,16 +49,16 @@ constexpr int CHU = 512;                 // units per ring slot (24 KB)
 constexpr int SLOT_BYTES = CHU * UNIT_BYTES;
 constexpr int NS_MAX = 8;                // ring slots (192 KB)
 constexpr int NS_MIN = 4;                // the reduction scratch aliases the first 4 slots (96 KB)
-constexpr int BAR_BYTES = 2 * NS_MAX * 8;
+constexpr int BAR_BYTES = (2 * NS_MAX + 4) * 8;
 constexpr int SMEM_MAX = 232448;         // 227 KB opt-in limit per CTA on sm_100
 constexpr int PAD_UNITS = CHU;           // dummy units appended to every system's stream
-constexpr int STATE_BYTES_PER_ROW = 12 * 8 + 8;  // X_n, X of the stage, V1, F (3 doubles each) + (phase, L) per dumbbell = 16 B / 2 rows
-constexpr int PROBE_SLOTS = 16;
+constexpr int STATE_BYTES_PER_ROW = 15 * 8 + 8;  // X_n, X of the stage (FP64 and rounded to T), V1, F (3 x 8 B each) + (phase, L) per dumbbell = 16 B / 2 rows
+constexpr int PROBE_SLOTS = 32;
 
 struct RunArgs {
     // problem
     int N, NQ, U, n_cta;      // spheres, quads = ceil(N/4), units = ceil(N/W), row tiles per system
-    int ns;                   // ring slots in use (NS_MIN..NS_MAX)
+    int buf_bytes;            // shared-memory stream buffer (multiple of 128, >= NS_MIN slots)
     int b0;                   // first system of this launch (blockIdx.y is relative to it)
     long long unit_stride;    // units per system in the streams (>= U + PAD_UNITS)
     void *units[2];           // beta-streams T[B][unit_stride][6][W]; stage g reads units[(cur+g)&1]
@@ -67,6 +67,7 @@ struct RunArgs {
     double self_mob;  // 1/(6 pi eta a)   Eq. (3a)
     double pre;       // 1/(8 pi eta)     Eq. (3b)
     double c1, c2;    // 2a^2/3, 2a^2     second line of Eq. (3b), see pair body
+    float c1f, c2f;   // the same rounded to FP32 on the host (no FP64 -> FP32 conversion in the pair loop)
     // what to run
     int mode;                 // RunMode
     int heun;                 // RUN_STEP: 1 = Heun (2 stages per step), 0 = Euler
@@ -126,10 +127,19 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async_global() { asm volatile("fence.proxy.async.global;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async_shared() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-__device__ __forceinline__ unsigned long long ld_acquire_gpu(const unsigned long long *p) {
+__device__ __forceinline__ unsigned long long ld_relaxed_gpu(const unsigned long long *p) {
     unsigned long long v;
-    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
     return v;
+}
+__device__ __forceinline__ void fence_acq_rel_gpu() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
+// Ampere-style asynchronous copy, 16 bytes global (L2 only, .cg) -> shared, in the generic proxy (SASS: LDGSTS);
+// the mbarrier form makes `bar` count this thread's arrival once all its earlier copies have landed
+__device__ __forceinline__ void cp_async16(void *dst, const void *src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_arrive(uint64_t *bar) {
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 __device__ __forceinline__ void red_release_gpu(unsigned long long *p, unsigned long long v) {
     asm volatile("red.release.gpu.global.add.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
@@ -143,39 +153,35 @@ __device__ __forceinline__ void red_release_gpu(unsigned long long *p, unsigned 
 // The common factor 1/(8 pi mu) is applied once per alpha in the epilogue.
 // FMA-pipe instruction count per pack: 3 sub + 3 (r^2) + 3 (r.F) + 2 + 6 = 17 (Oseen), 21 (RPY).
 template <typename T, int TENSOR, bool GUARD>
-__device__ __forceinline__ void pair_units(const V2<T> *__restrict__ p, int stride, int iters,
-                                           const typename Pack<T>::V (&xi)[QI][3],
-                                           typename Pack<T>::V (&acc)[QI][3], typename Pack<T>::V c1,
-                                           typename Pack<T>::V negc2) {
+__device__ __forceinline__ void pair_unit(const V2<T> *__restrict__ p, const typename Pack<T>::V (&xi)[QI][3],
+                                          typename Pack<T>::V (&acc)[QI][3], typename Pack<T>::V c1,
+                                          typename Pack<T>::V negc2) {
     typedef Pack<T> P;
     typedef typename P::V V;
-#pragma unroll 2
-    for (int r = 0; r < iters; ++r, p += stride) {
-        const V2<T> q0 = p[0], q1 = p[1], q2 = p[2];
-        const V xj = q0.a, yj = q0.b, zj = q1.a, fx = q1.b, fy = q2.a, fz = q2.b;
+    const V2<T> q0 = p[0], q1 = p[1], q2 = p[2];
+    const V xj = q0.a, yj = q0.b, zj = q1.a, fx = q1.b, fy = q2.a, fz = q2.b;
 #pragma unroll
-        for (int k = 0; k < QI; ++k) {
-            const V dx = P::sub(xi[k][0], xj), dy = P::sub(xi[k][1], yj), dz = P::sub(xi[k][2], zj);
-            const V r2 = P::fma(dz, dz, P::fma(dy, dy, P::mul(dx, dx)));
-            const V ri = P::template rsq<GUARD>(r2);
-            const V rf = P::fma(dz, fz, P::fma(dy, fy, P::mul(dx, fx)));
-            const V w = P::mul(ri, ri);
-            if (TENSOR == TENSOR_OSEEN) {
-                const V s2 = P::mul(rf, w);
-                const V tx = P::fma(s2, dx, fx), ty = P::fma(s2, dy, fy), tz = P::fma(s2, dz, fz);
-                acc[k][0] = P::fma(ri, tx, acc[k][0]);
-                acc[k][1] = P::fma(ri, ty, acc[k][1]);
-                acc[k][2] = P::fma(ri, tz, acc[k][2]);
-            } else {
-                const V ri3 = P::mul(ri, w);
-                const V ca = P::fma(c1, ri3, ri);
-                const V e = P::fma(negc2, w, P::bc(T(1)));
-                const V g = P::mul(rf, ri3);
-                const V cb = P::mul(g, e);
-                acc[k][0] = P::fma(cb, dx, P::fma(ca, fx, acc[k][0]));
-                acc[k][1] = P::fma(cb, dy, P::fma(ca, fy, acc[k][1]));
-                acc[k][2] = P::fma(cb, dz, P::fma(ca, fz, acc[k][2]));
-            }
+    for (int k = 0; k < QI; ++k) {
+        const V dx = P::sub(xi[k][0], xj), dy = P::sub(xi[k][1], yj), dz = P::sub(xi[k][2], zj);
+        const V r2 = P::fma(dz, dz, P::fma(dy, dy, P::mul(dx, dx)));
+        const V ri = P::template rsq<GUARD>(r2);
+        const V rf = P::fma(dz, fz, P::fma(dy, fy, P::mul(dx, fx)));
+        const V w = P::mul(ri, ri);
+        if (TENSOR == TENSOR_OSEEN) {
+            const V s2 = P::mul(rf, w);
+            const V tx = P::fma(s2, dx, fx), ty = P::fma(s2, dy, fy), tz = P::fma(s2, dz, fz);
+            acc[k][0] = P::fma(ri, tx, acc[k][0]);
+            acc[k][1] = P::fma(ri, ty, acc[k][1]);
+            acc[k][2] = P::fma(ri, tz, acc[k][2]);
+        } else {
+            const V ri3 = P::mul(ri, w);
+            const V ca = P::fma(c1, ri3, ri);
+            const V e = P::fma(negc2, w, P::bc(T(1)));
+            const V g = P::mul(rf, ri3);
+            const V cb = P::mul(g, e);
+            acc[k][0] = P::fma(cb, dx, P::fma(ca, fx, acc[k][0]));
+            acc[k][1] = P::fma(cb, dy, P::fma(ca, fy, acc[k][1]));
+            acc[k][2] = P::fma(cb, dz, P::fma(ca, fz, acc[k][2]));
         }
     }
 }
@@ -188,14 +194,20 @@ __device__ __forceinline__ double stroke_length(double t, double phi, double ell
     return __dadd_rn(ell, __dmul_rn(lambda, sin(__dadd_rn(__dmul_rn(omega, t), phi))));
 }
 //   n = (X_{2s+1} - X_{2s})/d, g = k0 (d - L), F_{2s} = +g n, F_{2s+1} = -g n   (F = -dU/dX)
+// 1/d comes from the refined reciprocal square root of pack.cuh (relative error < 2^-60, no division, no
+// slow path: d^2 is finite, positive, normal); d = d^2 (1/d) gets one correction step, which leaves it
+// within a rounding of sqrt(d^2): g = k0 (d - L) cancels, so d has to be that accurate.
 __device__ __forceinline__ void dumbbell_force(const double (&x0)[3], const double (&x1)[3], double L, double k0,
                                                double (&F0)[3]) {
     const double s0 = __dsub_rn(x1[0], x0[0]), s1 = __dsub_rn(x1[1], x0[1]), s2 = __dsub_rn(x1[2], x0[2]);
-    const double d = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(s0, s0), __dmul_rn(s1, s1)), __dmul_rn(s2, s2)));
-    const double g = __dmul_rn(k0, __dsub_rn(d, L));
-    F0[0] = __dmul_rn(g, __ddiv_rn(s0, d));
-    F0[1] = __dmul_rn(g, __ddiv_rn(s1, d));
-    F0[2] = __dmul_rn(g, __ddiv_rn(s2, d));
+    const double d2 = __fma_rn(s2, s2, __fma_rn(s1, s1, __dmul_rn(s0, s0)));
+    const double y = Pack<double>::rsq<false>(d2);
+    double d = __dmul_rn(d2, y);
+    d = __fma_rn(__fma_rn(-d, d, d2), __dmul_rn(0.5, y), d);
+    const double cf = __dmul_rn(__dmul_rn(k0, __dsub_rn(d, L)), y);
+    F0[0] = __dmul_rn(cf, s0);
+    F0[1] = __dmul_rn(cf, s1);
+    F0[2] = __dmul_rn(cf, s2);
 }
 // t_n = t0 + n dt, formed from the step index (never accumulated), no contraction
 __device__ __forceinline__ double time_of_step(double t0, long long n, double dt) {
@@ -241,13 +253,13 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
     constexpr int W = P::W;
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    const int ring_bytes = A.ns * SLOT_BYTES;
-    uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + ring_bytes);
+    const int buf_bytes = A.buf_bytes;   // stream buffer: the whole stage input if it fits (resident), else a ring of slots
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + buf_bytes);
     uint64_t *empty = full + NS_MAX;
+    uint64_t *gran = empty + NS_MAX;     // resident mode: one barrier per granule of the stream (3)
 
     const int tid = threadIdx.x, lane = tid & 31;
     const int c = blockIdx.x, b = A.b0 + blockIdx.y;
-    const int NS = A.ns;
 
     // rows of this CTA and the (alpha-thread, beta-group) shape
     const int q0 = (int)((long long)c * A.NQ / A.n_cta), q1 = (int)((long long)(c + 1) * A.NQ / A.n_cta);
@@ -255,37 +267,75 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
     const int n_jg = NT / nq;
     const int ith = tid % nq, jg = tid / nq;
     const bool active = jg < n_jg;
-    const int chu = (CHU / n_jg) * n_jg;    // units per chunk: a multiple of n_jg, <= CHU (n_jg <= NT = CHU)
-    const int nchunks = (A.U + chu - 1) / chu;
     const int rows = 4 * nq;
     const long long r0 = 4LL * q0;                                   // first sphere of this CTA
     const int nrows = (int)((A.N - r0) < rows ? (A.N - r0) : rows);  // real rows (N even in the step modes)
     const int nd = nrows >> 1;                                       // dumbbells owned (step modes)
     const size_t sys3 = (size_t)b * A.N * 3;
+    const bool stepping = A.mode != RUN_APPLY;
 
     // per-row state (step modes), FP64: X_n, Xc = positions the current stage evaluates (X_n or the
-    // predictor's X*), V1, F(Xc); per dumbbell: phase, L(t_{n+1})
+    // predictor's X*; XcT = the same rounded to T as the stream holds them), V1, F(Xc); per dumbbell: phase, L(t_{n+1})
     double *Xs, *Xc, *V1s, *Fs, *Ls;
+    T *XcT = nullptr;
     const double *phs;
     if (A.state_smem) {
-        double *st = reinterpret_cast<double *>(smem_raw + ring_bytes + BAR_BYTES);
+        double *st = reinterpret_cast<double *>(smem_raw + buf_bytes + BAR_BYTES);
         Xs = st; Xc = st + 3 * rows; V1s = st + 6 * rows; Fs = st + 9 * rows; Ls = st + 12 * rows;
         phs = st + 12 * rows + (rows >> 1);
+        XcT = reinterpret_cast<T *>(st + 13 * rows);
     } else {
         Xs = A.X + sys3 + 3 * r0; Xc = A.Xcg + sys3 + 3 * r0; V1s = A.V1g + sys3 + 3 * r0; Fs = A.Fg + sys3 + 3 * r0;
         Ls = A.Lg + (size_t)b * (A.N / 2) + (r0 >> 1);
         phs = A.phase + (size_t)b * (A.N / 2) + (r0 >> 1);
     }
 
+
+    // the stage's stream: total_it iterations of n_jg units each (tail padded with far-away zero-force units)
+    const int total_it = (A.U + n_jg - 1) / n_jg;
+    const int stride = 3 * n_jg;                               // 16-byte pieces per iteration
+    const int tp = total_it * stride;                          // pieces of the whole stream
+    const bool resident = (long long)tp * 16 <= buf_bytes;     // it fits: no ring, no refills
+    // resident mode.  The stream sits in shared memory in its natural order; the CTA consumes it starting at
+    // the iteration that holds its own rows (so only the first n_guard iterations need the r = 0 guard, and
+    // the 148 CTAs start at 148 different places of the L2-resident stream), wrapping around at the end.
+    // Three granules in consumption order, each with its own mbarrier: G0 (h0 iterations, copied first),
+    // G1 (h1), G2 (the rest, copied by the loop itself while it works on G0 and G1).
+    const int d0 = (4 * q0) / W, d1 = (4 * q1 + W - 1) / W;    // units that hold this CTA's own rows
+    const int it_own = d0 / n_jg;
+    const int n_guard = (d1 - 1) / n_jg - it_own + 1;
+    const int sp = it_own * stride;                            // first piece in consumption order
+    const int h0 = total_it < 3 ? total_it : 3;
+    const int h1 = total_it - h0 < 6 ? total_it - h0 : 6;
+    const int h2 = total_it - h0 - h1;
+    const int pA = h0 * stride, pAB = (h0 + h1) * stride;      // piece index (consumption order) where G1 / G2 start
+    // ring mode: chunks of cit iterations (<= one slot of CHU units)
+    const int NS = buf_bytes / SLOT_BYTES < NS_MAX ? buf_bytes / SLOT_BYTES : NS_MAX;
+    const int cit = CHU / n_jg;
+    const int chu = cit * n_jg;
+    const int nchunks = (total_it + cit - 1) / cit;
+    const int rot = c % nchunks;                               // CTAs start at different chunks: no L2 convoy
+
+    const V c1 = P::bc(sizeof(T) == 4 ? (T)A.c1f : (T)A.c1), negc2 = P::bc(sizeof(T) == 4 ? (T)(-A.c2f) : (T)(-A.c2));
+    // reduction shape (stage-invariant index arithmetic is done once, here)
+    const int n_out = 12 * nq;
+    int nparts = NT / n_out;
+    nparts = nparts < 1 ? 1 : (nparts > n_jg ? n_jg : nparts);
+    const int red_w = jg * n_out + ith;             // this thread's first partial in red[jg][o]
+    const int l2_o = tid % n_out, l2_part = tid / n_out;     // level-2 task of this thread (when n_out * nparts <= NT)
+
+
     if (tid == 0) {
-        for (int s = 0; s < NS; ++s) {
+        for (int s = 0; s < NS_MAX; ++s) {
             mbar_init(full + s, 1);
             mbar_init(empty + s, NT / 32);
         }
+        mbar_init(gran + 0, NT);   // G0, G1: every thread's LDGSTS copies
+        mbar_init(gran + 1, NT);
+        mbar_init(gran + 2, 1);    // G2: thread 0's TMA bulk copies
         mbar_fence_init();
     }
 
-    const bool stepping = A.mode != RUN_APPLY;
     const int n_stage = A.mode == RUN_STEP ? (int)(A.n_steps * (A.heun ? 2 : 1)) : 1;
     unsigned long long *bar = A.bar != nullptr ? A.bar + b : nullptr;
     unsigned long long bar_target = A.bar_base;
@@ -298,7 +348,10 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
             for (int sl = tid; sl < nd; sl += NT) const_cast<double *>(phs)[sl] = A.phase[(size_t)b * (A.N / 2) + (r0 >> 1) + sl];
         }
         __syncthreads();
-        for (int e = tid; e < 3 * nrows; e += NT) Xc[e] = Xs[e];
+        for (int e = tid; e < 3 * nrows; e += NT) {
+            Xc[e] = Xs[e];
+            if (XcT != nullptr) XcT[e] = (T)Xs[e];
+        }
         const double tn = time_of_step(A.t0, A.n0, A.dt);
         T *un = reinterpret_cast<T *>(A.units[A.cur]) + (size_t)b * A.unit_stride * (6 * W);
         for (int sl = tid; sl < nd; sl += NT) {
@@ -310,49 +363,39 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
             for (int cc = 0; cc < 3; ++cc) { Fs[6 * sl + cc] = F0[cc]; Fs[6 * sl + 3 + cc] = -F0[cc]; }
             publish_dumbbell(un, r0 + 2 * sl, x0, x1, F0);
         }
-        fence_proxy_async_global();
+        fence_proxy_async_global();   // the stream is also read through the async proxy (TMA)
     }
     __syncthreads();  // mbarriers initialised; state and published rows written
 
-    uint32_t seq0 = 0;  // chunk sequence number of the stage's first chunk (slot = seq % NS, parity = (seq / NS) & 1)
-    for (int g = 0; g < n_stage; ++g, seq0 += (uint32_t)nchunks) {
+
+    // ring mode: k-th chunk in this CTA's consumption order -> chunk index, iterations; ring position of the next
+    // chunk to consume / to fill (slot, and how often the ring has been gone around: fill parity = wraps & 1)
+    auto chunk_of = [&](int k) { const int ch = k + rot; return ch >= nchunks ? ch - nchunks : ch; };
+    auto chunk_iters = [&](int ch) { const int rem = total_it - ch * cit; return rem < cit ? rem : cit; };
+    int cslot = 0, pslot = 0;
+    uint32_t cwraps = 0, pwraps = 0;
+
+    for (int g = 0; g < n_stage; ++g) {
         probe_on = (g == n_stage - 1);
         DS_PROBE(0);
         const T *units = reinterpret_cast<const T *>(A.units[(A.cur + g) & 1]) + (size_t)b * A.unit_stride * (6 * W);
-        const int n_pre = nchunks < NS ? nchunks : NS;  // chunks in flight before the loop starts
 
-        // chunk ch = units [ch chu, ch chu + cu): cu rounded up to a multiple of n_jg (the pad units exist)
-        auto chunk_units = [&](int ch) {
-            const int rem = A.U - ch * chu;
-            return rem >= chu ? chu : (rem + n_jg - 1) / n_jg * n_jg;
-        };
-        auto issue = [&](int ch) {
-            const uint32_t seq = seq0 + (uint32_t)ch;
-            const int s = (int)(seq % (uint32_t)NS);
-            if (seq >= (uint32_t)NS) mbar_wait(empty + s, ((seq / (uint32_t)NS) - 1u) & 1u);  // previous content consumed
-            const uint32_t bytes = (uint32_t)chunk_units(ch) * UNIT_BYTES;
-            mbar_expect_tx(full + s, bytes);
-            bulk_g2s(smem_raw + (size_t)s * SLOT_BYTES, units + (size_t)ch * chu * (6 * W), bytes, full + s);
-        };
-
-        if (tid == 0) {
-            if (stepping && A.n_cta > 1) {
-                // inter-CTA barrier: every CTA of the system has published its rows of this stage's input
-                __threadfence();
-                red_release_gpu(bar, 1ULL);
-                bar_target += (unsigned long long)A.n_cta;
-                while (ld_acquire_gpu(bar) < bar_target) {}
-            }
-            DS_PROBE(1);
-            fence_proxy_async();
-            for (int ch = 0; ch < n_pre; ++ch) issue(ch);
+        if (tid == 0 && stepping && A.n_cta > 1) {
+            // inter-CTA barrier: every CTA of the system has published its rows of this stage's input
+            red_release_gpu(bar, 1ULL);
+            DS_PROBE(12);
+            bar_target += (unsigned long long)A.n_cta;
+            while (ld_relaxed_gpu(bar) < bar_target) {}
+            fence_acq_rel_gpu();
         }
-
+        DS_PROBE(1);
         // stroke length at the end of this step, L(t_{n+1}), once per step (warps 1.. while warp 0 waits)
         if (A.mode == RUN_STEP && (!A.heun || (g & 1) == 0) && tid >= 32) {
             const double t1 = time_of_step(A.t0, A.n0 + (A.heun ? (g >> 1) : g) + 1, A.dt);
             for (int sl = tid - 32; sl < nd; sl += NT - 32) Ls[sl] = stroke_length(t1, phs[sl], A.ell, A.lambda, A.omega);
         }
+        if (stepping && A.n_cta > 1) __syncthreads();   // the barrier has been passed (thread 0)
+        DS_PROBE(9);
 
         // alpha-spheres of this thread: rows 4 (q0 + ith) + k, rounded exactly as the stream rounds them
         V xi[QI][3], acc[QI][3];
@@ -361,113 +404,198 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
             const int il = 4 * ith + k;
             T x = T(0), y = T(0), z = T(0);
             if (il < nrows) {
-                if (stepping) {
-                    x = (T)Xc[3 * il]; y = (T)Xc[3 * il + 1]; z = (T)Xc[3 * il + 2];
+                if (XcT != nullptr && stepping) {
+                    x = XcT[3 * il]; y = XcT[3 * il + 1]; z = XcT[3 * il + 2];
                 } else {
-                    x = __ldg(units + unit_index<T>(r0 + il, 0));
-                    y = __ldg(units + unit_index<T>(r0 + il, 1));
-                    z = __ldg(units + unit_index<T>(r0 + il, 2));
+                    x = __ldcg(units + unit_index<T>(r0 + il, 0));
+                    y = __ldcg(units + unit_index<T>(r0 + il, 1));
+                    z = __ldcg(units + unit_index<T>(r0 + il, 2));
                 }
             }
             xi[k][0] = P::bc(x); xi[k][1] = P::bc(y); xi[k][2] = P::bc(z);
             acc[k][0] = acc[k][1] = acc[k][2] = P::bc(T(0));
         }
-        const V c1 = P::bc((T)A.c1), negc2 = P::bc((T)(-A.c2));
-        const int d0 = (4 * q0) / W, d1 = (4 * q1 + W - 1) / W;  // units that hold this CTA's own rows
+        DS_PROBE(11);
 
-        for (int ch = 0; ch < nchunks; ++ch) {
-            const uint32_t seq = seq0 + (uint32_t)ch;
-            const int s = (int)(seq % (uint32_t)NS);
-            mbar_wait(full + s, (seq / (uint32_t)NS) & 1u);
-            if (ch == 0) DS_PROBE(2);
-            if (active) {
-                const int u0 = ch * chu, cu = chunk_units(ch);
-                const V2<T> *p = reinterpret_cast<const V2<T> *>(smem_raw + (size_t)s * SLOT_BYTES) + 3 * jg;
-                if (u0 < d1 && u0 + cu > d0)
-                    pair_units<T, TENSOR, true>(p, 3 * n_jg, cu / n_jg, xi, acc, c1, negc2);
-                else
-                    pair_units<T, TENSOR, false>(p, 3 * n_jg, cu / n_jg, xi, acc, c1, negc2);
+
+        if (resident) {
+            // ---- resident stream: LDGSTS copies (generic proxy, L2 -> shared, 16 bytes per thread and piece) ----
+            const uint4 *gsrc = reinterpret_cast<const uint4 *>(units);
+            uint4 *sdst = reinterpret_cast<uint4 *>(smem_raw);
+            auto copy_piece = [&](int j) {          // j-th piece in consumption order
+                int a = sp + j;
+                a = a >= tp ? a - tp : a;
+                cp_async16(sdst + a, gsrc + a);
+            };
+            const uint32_t par = (uint32_t)g & 1u;  // every granule barrier completes one phase per stage
+            if (tid == 0 && h2 > 0) {               // G2: one TMA bulk copy (two if it wraps around the end of the stream)
+                int a0 = sp + pAB;
+                a0 = a0 >= tp ? a0 - tp : a0;
+                const int len = tp - pAB, first = a0 + len <= tp ? len : tp - a0;
+                mbar_expect_tx(gran + 2, (uint32_t)len * 16u);
+                bulk_g2s(sdst + a0, gsrc + a0, (uint32_t)first * 16u, gran + 2);
+                if (first < len) bulk_g2s(sdst, gsrc, (uint32_t)(len - first) * 16u, gran + 2);
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(empty + s);                 // this warp is done with the slot
-            if (tid == 0 && ch + NS < nchunks) issue(ch + NS);     // refill it once every warp is
+            for (int j = tid; j < pA; j += NT) copy_piece(j);
+            cp_async_arrive(gran + 0);
+            if (h1 > 0) {
+                for (int j = pA + tid; j < pAB; j += NT) copy_piece(j);
+                cp_async_arrive(gran + 1);
+            }
+            DS_PROBE(10);
+            const V2<T> *const base = reinterpret_cast<const V2<T> *>(smem_raw) + 3 * jg;
+            mbar_wait(gran + 0, par);
+            DS_PROBE(2);
+            // the stage's total_it iterations (each: QI alpha x 1 unit per thread) as a few tight loops: a new one
+            // starts where a granule begins, where the guard ends and where the stream wraps around
+            const int ng = n_guard <= h0 ? h0 : n_guard, wrapq = total_it - it_own;
+            int q = 0;
+            while (q < total_it) {
+                if (q == h0 && h1 > 0) mbar_wait(gran + 1, par);
+                if (q == h0 + h1 && h2 > 0) mbar_wait(gran + 2, par);
+                int qe = q < h0 ? h0 : (q < h0 + h1 ? h0 + h1 : total_it);
+                if (q < ng && ng < qe) qe = ng;
+                if (q < wrapq && wrapq < qe) qe = wrapq;
+                if (active) {
+                    int it = it_own + q;
+                    it = it >= total_it ? it - total_it : it;
+                    const V2<T> *p = base + it * stride;
+                    if (q < ng) {
+#pragma unroll 1
+                        for (int r = q; r < qe; ++r, p += stride) pair_unit<T, TENSOR, true>(p, xi, acc, c1, negc2);
+                    } else {
+#pragma unroll 2
+                        for (int r = q; r < qe; ++r, p += stride) pair_unit<T, TENSOR, false>(p, xi, acc, c1, negc2);
+                    }
+                }
+                q = qe;
+            }
+        } else {
+            // ---- ring of slots filled by TMA bulk copies (thread 0), one tight loop per chunk ----
+            auto issue_tma = [&](int k) {
+                const int ch = chunk_of(k);
+                if (pwraps > 0) mbar_wait(empty + pslot, (pwraps - 1u) & 1u);   // previous content consumed by every warp
+                const uint32_t bytes = (uint32_t)(chunk_iters(ch) * n_jg) * UNIT_BYTES;
+                mbar_expect_tx(full + pslot, bytes);
+                bulk_g2s(smem_raw + (size_t)pslot * SLOT_BYTES, units + (size_t)ch * chu * (6 * W), bytes, full + pslot);
+                if (++pslot == NS) { pslot = 0; ++pwraps; }
+            };
+            if (tid == 0) {
+                fence_proxy_async();
+                for (int k = 0; k < NS && k < nchunks; ++k) issue_tma(k);
+            }
+            DS_PROBE(10);
+            for (int k = 0; k < nchunks; ++k) {
+                const int ch = chunk_of(k);
+                mbar_wait(full + cslot, cwraps & 1u);
+                if (k == 0) DS_PROBE(2);
+                if (active) {
+                    const int u0 = ch * chu, its = chunk_iters(ch);
+                    const V2<T> *p = reinterpret_cast<const V2<T> *>(smem_raw + (size_t)cslot * SLOT_BYTES) + 3 * jg;
+                    if (u0 < d1 && u0 + its * n_jg > d0) {
+#pragma unroll 1
+                        for (int r = 0; r < its; ++r, p += stride) pair_unit<T, TENSOR, true>(p, xi, acc, c1, negc2);
+                    } else {
+#pragma unroll 2
+                        for (int r = 0; r < its; ++r, p += stride) pair_unit<T, TENSOR, false>(p, xi, acc, c1, negc2);
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty + cslot);                 // this warp is done with the slot
+                if (tid == 0 && k + NS < nchunks) issue_tma(k + NS);       // refill it once every warp is
+                if (++cslot == NS) { cslot = 0; ++cwraps; }
+            }
         }
+
         DS_PROBE(3);
         __syncthreads();  // every chunk consumed by every warp: the ring is free and becomes scratch
         DS_PROBE(4);
 
-        // ---- sum over the n_jg beta-groups (fixed order) ----
+        // ---- sum over the n_jg beta-groups (fixed order): red[jg][o] -> red2[part][o] ----
         T *red = reinterpret_cast<T *>(smem_raw);   // [n_jg][n_out]   <= 12 NT
         T *red2 = red + 12 * NT;                    // [nparts][n_out] <= 12 NT     (2 x 12 NT x 8 B = 96 KB = NS_MIN slots)
-        const int n_out = 12 * nq;
         if (active) {
 #pragma unroll
             for (int k = 0; k < QI; ++k)
 #pragma unroll
-                for (int cc = 0; cc < 3; ++cc) red[(size_t)jg * n_out + (k * 3 + cc) * nq + ith] = P::hsum(acc[k][cc]);
+                for (int cc = 0; cc < 3; ++cc) red[red_w + (k * 3 + cc) * nq] = P::hsum(acc[k][cc]);
         }
         __syncthreads();
-        int nparts = NT / n_out;
-        nparts = nparts < 1 ? 1 : (nparts > n_jg ? n_jg : nparts);
-        for (int idx = tid; idx < n_out * nparts; idx += NT) {
-            const int o = idx % n_out, part = idx / n_out;
-            T sum = T(0);
-            for (int gq = part; gq < n_jg; gq += nparts) sum += red[(size_t)gq * n_out + o];
-            red2[(size_t)part * n_out + o] = sum;
+        if (nparts > 1) {            // n_out * nparts <= NT: one (o, part) task per thread
+            if (l2_part < nparts) {
+                const T *rp = red + l2_o;
+                T sa = T(0), sb = T(0);
+                int gq = l2_part;
+                for (; gq + nparts < n_jg; gq += 2 * nparts) {
+                    sa += rp[gq * n_out];
+                    sb += rp[(gq + nparts) * n_out];
+                }
+                if (gq < n_jg) sa += rp[gq * n_out];
+                red2[l2_part * n_out + l2_o] = sa + sb;
+            }
+        } else {                     // one part: thread o sums all groups
+            for (int o = tid; o < n_out; o += NT) {
+                T sa = T(0), sb = T(0);
+                int gq = 0;
+                for (; gq + 1 < n_jg; gq += 2) {
+                    sa += red[gq * n_out + o];
+                    sb += red[(gq + 1) * n_out + o];
+                }
+                if (gq < n_jg) sa += red[gq * n_out + o];
+                red2[o] = sa + sb;
+            }
         }
         __syncthreads();
         DS_PROBE(5);
-        // u of local row il, component cc: the parts are added in FP64, then Eq. (3a) + the 1/(8 pi mu) factor
-        auto velocity = [&](int il, int cc, double Fi) {
-            const int o = ((il & 3) * 3 + cc) * nq + (il >> 2);
-            double sum = (double)red2[o];
-            for (int part = 1; part < nparts; ++part) sum += (double)red2[(size_t)part * n_out + o];
-            return A.self_mob * Fi + A.pre * sum;
+        // u of state element e = 3 il + cc (local row il, component cc): the parts are added, then Eq. (3a)
+        // and the 1/(8 pi mu) factor in FP64
+        auto velocity = [&](int e, double Fi) {
+            const int il = e / 3, cc = e - 3 * il;
+            const T *rp = red2 + ((il & 3) * 3 + cc) * nq + (il >> 2);
+            T sum = rp[0];
+            for (int part = 1; part < nparts; ++part) sum += rp[part * n_out];
+            return A.self_mob * Fi + A.pre * (double)sum;
         };
 
         if (!stepping) {  // ---- RUN_APPLY: a2 + a3 with the stream's own F ----
-            for (int il = tid; il < nrows; il += NT) {
-                const long long i = r0 + il;
-#pragma unroll
-                for (int cc = 0; cc < 3; ++cc)
-                    reinterpret_cast<T *>(A.out_u)[(size_t)i * 3 + cc] = (T)velocity(il, cc, (double)units[unit_index<T>(i, 3 + cc)]);
+            for (int e = tid; e < 3 * nrows; e += NT) {
+                const long long i = r0 + e / 3;
+                reinterpret_cast<T *>(A.out_u)[(size_t)3 * r0 + e] = (T)velocity(e, (double)units[unit_index<T>(i, 3 + e % 3)]);
             }
         } else if (A.mode == RUN_VELOCITY) {
-            for (int il = tid; il < nrows; il += NT)
-#pragma unroll
-                for (int cc = 0; cc < 3; ++cc)
-                    reinterpret_cast<T *>(A.out_u)[sys3 + (size_t)(r0 + il) * 3 + cc] = (T)velocity(il, cc, Fs[3 * il + cc]);
-        } else {  // ---- RUN_STEP: integrator, Eq. (4) at the new positions, publish ----
+            for (int e = tid; e < 3 * nrows; e += NT)
+                reinterpret_cast<T *>(A.out_u)[sys3 + (size_t)3 * r0 + e] = (T)velocity(e, Fs[e]);
+        } else {  // ---- RUN_STEP: integrator, one thread per state element ----
             const bool pred = A.heun && (g & 1) == 0, corr = A.heun && (g & 1) == 1;
+            for (int e = tid; e < 3 * nrows; e += NT) {
+                const double v = velocity(e, Fs[e]);
+                double xn;
+                if (pred) {            // X* = X_n + dt V1
+                    V1s[e] = v;
+                    xn = Xs[e] + A.dt * v;
+                } else if (corr) {     // X_{n+1} = X_n + (dt/2)(V1 + V2)
+                    xn = Xs[e] + (0.5 * A.dt) * (V1s[e] + v);
+                    Xs[e] = xn;
+                } else {               // Euler
+                    xn = Xs[e] + A.dt * v;
+                    Xs[e] = xn;
+                }
+                Xc[e] = xn;
+                if (XcT != nullptr) XcT[e] = (T)xn;
+            }
+            __syncthreads();
+            // Eq. (4) at the new positions and time, one thread per dumbbell; publish the next stage's rows
             T *un = reinterpret_cast<T *>(A.units[(A.cur + g + 1) & 1]) + (size_t)b * A.unit_stride * (6 * W);
             for (int sl = tid; sl < nd; sl += NT) {
-                double xs[2][3], F0[3];
+                double x0[3], x1[3], F0[3];
 #pragma unroll
-                for (int r = 0; r < 2; ++r)
-#pragma unroll
-                    for (int cc = 0; cc < 3; ++cc) {
-                        const int e = 3 * (2 * sl + r) + cc;
-                        const double v = velocity(2 * sl + r, cc, Fs[e]);
-                        double xn;
-                        if (pred) {            // X* = X_n + dt V1
-                            V1s[e] = v;
-                            xn = Xs[e] + A.dt * v;
-                        } else if (corr) {     // X_{n+1} = X_n + (dt/2)(V1 + V2)
-                            xn = Xs[e] + (0.5 * A.dt) * (V1s[e] + v);
-                            Xs[e] = xn;
-                        } else {               // Euler
-                            xn = Xs[e] + A.dt * v;
-                            Xs[e] = xn;
-                        }
-                        xs[r][cc] = xn;
-                        Xc[e] = xn;
-                    }
-                dumbbell_force(xs[0], xs[1], Ls[sl], A.k0, F0);
+                for (int cc = 0; cc < 3; ++cc) { x0[cc] = Xc[6 * sl + cc]; x1[cc] = Xc[6 * sl + 3 + cc]; }
+                dumbbell_force(x0, x1, Ls[sl], A.k0, F0);
 #pragma unroll
                 for (int cc = 0; cc < 3; ++cc) { Fs[6 * sl + cc] = F0[cc]; Fs[6 * sl + 3 + cc] = -F0[cc]; }
-                if (g + 1 < n_stage) publish_dumbbell(un, r0 + 2 * sl, xs[0], xs[1], F0);
+                if (g + 1 < n_stage) publish_dumbbell(un, r0 + 2 * sl, x0, x1, F0);
             }
-            fence_proxy_async_global();
+            fence_proxy_async_global();   // the stream is also read through the async proxy (TMA)
         }
         DS_PROBE(6);
         fence_proxy_async_shared();
