@@ -305,7 +305,7 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
     const int it_own = d0 / n_jg;
     const int n_guard = (d1 - 1) / n_jg - it_own + 1;
     const int sp = it_own * stride;                            // first piece in consumption order
-    const int h0 = total_it < 3 ? total_it : 3;
+    const int h0 = total_it < 4 ? total_it : 4;
     const int h1 = total_it - h0 < 6 ? total_it - h0 : 6;
     const int h2 = total_it - h0 - h1;
     const int pA = h0 * stride, pAB = (h0 + h1) * stride;      // piece index (consumption order) where G1 / G2 start
@@ -330,9 +330,9 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
             mbar_init(full + s, 1);
             mbar_init(empty + s, NT / 32);
         }
-        mbar_init(gran + 0, NT);   // G0, G1: every thread's LDGSTS copies
-        mbar_init(gran + 1, NT);
-        mbar_init(gran + 2, 1);    // G2: thread 0's TMA bulk copies
+        mbar_init(gran + 0, NT);   // G0: every thread's LDGSTS copies
+        mbar_init(gran + 1, 1);    // G1, G2: thread 0's TMA bulk copies
+        mbar_init(gran + 2, 1);
         mbar_fence_init();
     }
 
@@ -428,45 +428,52 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
                 cp_async16(sdst + a, gsrc + a);
             };
             const uint32_t par = (uint32_t)g & 1u;  // every granule barrier completes one phase per stage
-            if (tid == 0 && h2 > 0) {               // G2: one TMA bulk copy (two if it wraps around the end of the stream)
-                int a0 = sp + pAB;
-                a0 = a0 >= tp ? a0 - tp : a0;
-                const int len = tp - pAB, first = a0 + len <= tp ? len : tp - a0;
-                mbar_expect_tx(gran + 2, (uint32_t)len * 16u);
-                bulk_g2s(sdst + a0, gsrc + a0, (uint32_t)first * 16u, gran + 2);
-                if (first < len) bulk_g2s(sdst, gsrc, (uint32_t)(len - first) * 16u, gran + 2);
+            if (tid == 0) {   // G1, G2: TMA bulk copies of consumption pieces [j0, j1) (two copies where the range wraps)
+                auto tma_range = [&](int j0, int j1, uint64_t *bar) {
+                    int a0 = sp + j0;
+                    a0 = a0 >= tp ? a0 - tp : a0;
+                    const int len = j1 - j0, first = a0 + len <= tp ? len : tp - a0;
+                    mbar_expect_tx(bar, (uint32_t)len * 16u);
+                    bulk_g2s(sdst + a0, gsrc + a0, (uint32_t)first * 16u, bar);
+                    if (first < len) bulk_g2s(sdst, gsrc, (uint32_t)(len - first) * 16u, bar);
+                };
+                if (h1 > 0) tma_range(pA, pAB, gran + 1);
+                if (h2 > 0) tma_range(pAB, tp, gran + 2);
             }
-            for (int j = tid; j < pA; j += NT) copy_piece(j);
+            for (int j = tid; j < pA; j += NT) copy_piece(j);   // G0: LDGSTS by every thread (lowest latency)
             cp_async_arrive(gran + 0);
-            if (h1 > 0) {
-                for (int j = pA + tid; j < pAB; j += NT) copy_piece(j);
-                cp_async_arrive(gran + 1);
-            }
             DS_PROBE(10);
             const V2<T> *const base = reinterpret_cast<const V2<T> *>(smem_raw) + 3 * jg;
             mbar_wait(gran + 0, par);
             DS_PROBE(2);
             // the stage's total_it iterations (each: QI alpha x 1 unit per thread) as a few tight loops: a new one
             // starts where a granule begins, where the guard ends and where the stream wraps around
-            const int ng = n_guard <= h0 ? h0 : n_guard, wrapq = total_it - it_own;
+            const int wrapq = total_it - it_own;
             int q = 0;
             while (q < total_it) {
-                if (q == h0 && h1 > 0) mbar_wait(gran + 1, par);
-                if (q == h0 + h1 && h2 > 0) mbar_wait(gran + 2, par);
+                if (q == h0 && h1 > 0) { DS_PROBE(13); mbar_wait(gran + 1, par); DS_PROBE(14); }
+                if (q == h0 + h1 && h2 > 0) { DS_PROBE(15); mbar_wait(gran + 2, par); DS_PROBE(16); }
                 int qe = q < h0 ? h0 : (q < h0 + h1 ? h0 + h1 : total_it);
-                if (q < ng && ng < qe) qe = ng;
+                if (q < n_guard && n_guard < qe) qe = n_guard;
                 if (q < wrapq && wrapq < qe) qe = wrapq;
-                if (active) {
-                    int it = it_own + q;
-                    it = it >= total_it ? it - total_it : it;
-                    const V2<T> *p = base + it * stride;
-                    if (q < ng) {
+                int it = it_own + q;
+                it = it >= total_it ? it - total_it : it;
+                const V2<T> *p = base + it * stride;
+                if (q < n_guard) {
+                    // iterations that hold the CTA's own rows: a warp takes the guarded variant (r = 0 excluded)
+                    // only if one of its lanes reads an own unit in that iteration
+                    int u = it * n_jg + jg;
 #pragma unroll 1
-                        for (int r = q; r < qe; ++r, p += stride) pair_unit<T, TENSOR, true>(p, xi, acc, c1, negc2);
-                    } else {
-#pragma unroll 2
-                        for (int r = q; r < qe; ++r, p += stride) pair_unit<T, TENSOR, false>(p, xi, acc, c1, negc2);
+                    for (int r = q; r < qe; ++r, p += stride, u += n_jg) {
+                        const bool own = __any_sync(0xffffffffu, active && u >= d0 && u < d1);
+                        if (active) {
+                            if (own) pair_unit<T, TENSOR, true>(p, xi, acc, c1, negc2);
+                            else pair_unit<T, TENSOR, false>(p, xi, acc, c1, negc2);
+                        }
                     }
+                } else if (active) {
+#pragma unroll 2
+                    for (int r = q; r < qe; ++r, p += stride) pair_unit<T, TENSOR, false>(p, xi, acc, c1, negc2);
                 }
                 q = qe;
             }
