@@ -169,9 +169,21 @@ int choose_shape_step(ds_system *s) {
     return DS_OK;
 }
 
-template <typename T, int TENSOR>
-int launch_run_t(ds_system *s, ds::RunArgs &A, dim3 grid, size_t smem, bool coop, cudaStream_t st) {
-    auto kern = ds::run_kernel<T, TENSOR>;
+// The stream of a launch is resident when every CTA's padded stream (iterations x groups x 48 B) fits the buffer;
+// CTAs own floor or ceil(NQ / n_cta) quads, hence two shapes to check.
+bool stream_resident(int NQ, int U, int n_cta, int buf_bytes) {
+    const int nq_lo = NQ / n_cta, nq_hi = (NQ + n_cta - 1) / n_cta;
+    for (int nq = nq_lo < 1 ? 1 : nq_lo; nq <= nq_hi; ++nq) {
+        const int n_jg = ds::NT / nq;
+        const long long total_it = (U + n_jg - 1) / n_jg;
+        if (total_it * n_jg * ds::UNIT_BYTES > buf_bytes) return false;
+    }
+    return true;
+}
+
+template <typename T, int TENSOR, int MODE, bool RES>
+int launch_run_v(ds_system *s, ds::RunArgs &A, dim3 grid, size_t smem, bool coop, cudaStream_t st) {
+    auto kern = ds::run_kernel<T, TENSOR, MODE, RES>;
     static bool attr_done = false;
     if (!attr_done) {
         CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, ds::SMEM_MAX));
@@ -186,6 +198,24 @@ int launch_run_t(ds_system *s, ds::RunArgs &A, dim3 grid, size_t smem, bool coop
     }
     s->launches += 1;
     return DS_OK;
+}
+
+template <typename T, int TENSOR>
+int launch_run_t(ds_system *s, ds::RunArgs &A, dim3 grid, size_t smem, bool coop, cudaStream_t st) {
+    const int km = A.mode == ds::RUN_APPLY ? ds::KM_APPLY : A.mode == ds::RUN_VELOCITY ? ds::KM_VELOCITY
+                 : A.heun ? ds::KM_HEUN : ds::KM_EULER;
+    const bool res = stream_resident(A.NQ, A.U, A.n_cta, A.buf_bytes);
+#define DS_CASE(M)                                                                      \
+    case M: return res ? launch_run_v<T, TENSOR, M, true>(s, A, grid, smem, coop, st)   \
+                       : launch_run_v<T, TENSOR, M, false>(s, A, grid, smem, coop, st);
+    switch (km) {
+        DS_CASE(ds::KM_APPLY)
+        DS_CASE(ds::KM_VELOCITY)
+        DS_CASE(ds::KM_EULER)
+        DS_CASE(ds::KM_HEUN)
+    }
+#undef DS_CASE
+    return DS_ERR_INVALID_PARAM;
 }
 
 int launch_run(ds_system *s, ds::RunArgs &A, dim3 grid, size_t smem, bool coop, cudaStream_t st) {

@@ -41,6 +41,8 @@ namespace ds {
 
 enum { TENSOR_OSEEN = 0, TENSOR_RPY = 1 };
 enum RunMode { RUN_APPLY = 0, RUN_VELOCITY = 1, RUN_STEP = 2 };
+// kernel variants (template parameter): the stage's tail is compiled for one of these only
+enum KernelMode { KM_APPLY = 0, KM_VELOCITY = 1, KM_EULER = 2, KM_HEUN = 3 };
 
 constexpr int NT = 512;                  // threads per CTA: 16 warps, one CTA per SM
 constexpr int QI = 4;                    // alpha-spheres per thread (one quad)
@@ -239,14 +241,18 @@ __device__ __forceinline__ void publish_dumbbell(double *un, long long i0, const
     p[5] = make_double2(-F0[1], -F0[2]);
 }
 
+#ifdef DS_ENABLE_PROBE
 #define DS_PROBE(slot)                                                                          \
     do {                                                                                        \
         if (A.probe != nullptr && tid == 0 && probe_on)                                         \
             A.probe[((size_t)blockIdx.y * gridDim.x + blockIdx.x) * PROBE_SLOTS + (slot)] = clock64(); \
     } while (0)
+#else
+#define DS_PROBE(slot) do { } while (0)
+#endif
 
 // ---------------------------------------------------------------------------------------------
-template <typename T, int TENSOR>
+template <typename T, int TENSOR, int MODE, bool RESIDENT>
 __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
     typedef Pack<T> P;
     typedef typename P::V V;
@@ -272,7 +278,7 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
     const int nrows = (int)((A.N - r0) < rows ? (A.N - r0) : rows);  // real rows (N even in the step modes)
     const int nd = nrows >> 1;                                       // dumbbells owned (step modes)
     const size_t sys3 = (size_t)b * A.N * 3;
-    const bool stepping = A.mode != RUN_APPLY;
+    constexpr bool stepping = MODE != KM_APPLY;
 
     // per-row state (step modes), FP64: X_n, Xc = positions the current stage evaluates (X_n or the
     // predictor's X*; XcT = the same rounded to T as the stream holds them), V1, F(Xc); per dumbbell: phase, L(t_{n+1})
@@ -295,7 +301,7 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
     const int total_it = (A.U + n_jg - 1) / n_jg;
     const int stride = 3 * n_jg;                               // 16-byte pieces per iteration
     const int tp = total_it * stride;                          // pieces of the whole stream
-    const bool resident = (long long)tp * 16 <= buf_bytes;     // it fits: no ring, no refills
+    // RESIDENT: the host checked tp * 16 <= buf_bytes (no ring, no refills)
     // resident mode.  The stream sits in shared memory in its natural order; the CTA consumes it starting at
     // the iteration that holds its own rows (so only the first n_guard iterations need the r = 0 guard, and
     // the 148 CTAs start at 148 different places of the L2-resident stream), wrapping around at the end.
@@ -318,13 +324,13 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
 
     const V c1 = P::bc(sizeof(T) == 4 ? (T)A.c1f : (T)A.c1), negc2 = P::bc(sizeof(T) == 4 ? (T)(-A.c2f) : (T)(-A.c2));
     // reduction shape (stage-invariant index arithmetic is done once, here)
-    const int n_out = 12 * nq;
-    int nparts = NT / n_out;
-    nparts = nparts < 1 ? 1 : (nparts > n_jg ? n_jg : nparts);
-    const int red_w = jg * n_out + ith;             // this thread's first partial in red[jg][o]
-    const int l2_o = tid % n_out, l2_part = tid / n_out;     // level-2 task of this thread (when n_out * nparts <= NT)
-
-
+    // split-beta reduction: the partials of thread tid sit at red[12 tid + m], m = 3 k + cc (three 16-byte stores,
+    // 48-byte thread stride: conflict-free); the sums of quad ith are elements 12 ith + m of the CTA's state.
+    // A task = (quad ith, 4 consecutive m) is summed by RP consecutive lanes: lane part adds the groups
+    // jg = part, part + RP, ... with one LDS.128 each, then log2(RP) shuffle steps.
+    constexpr int RP = 8;
+    const int n_task = 3 * nq;                                  // tasks of the CTA
+    const int my_task = tid / RP, my_part = tid % RP;
     if (tid == 0) {
         for (int s = 0; s < NS_MAX; ++s) {
             mbar_init(full + s, 1);
@@ -336,7 +342,7 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
         mbar_fence_init();
     }
 
-    const int n_stage = A.mode == RUN_STEP ? (int)(A.n_steps * (A.heun ? 2 : 1)) : 1;
+    const int n_stage = MODE >= KM_EULER ? (int)(A.n_steps * (MODE == KM_HEUN ? 2 : 1)) : 1;
     unsigned long long *bar = A.bar != nullptr ? A.bar + b : nullptr;
     unsigned long long bar_target = A.bar_base;
     bool probe_on = false;
@@ -390,8 +396,8 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
         }
         DS_PROBE(1);
         // stroke length at the end of this step, L(t_{n+1}), once per step (warps 1.. while warp 0 waits)
-        if (A.mode == RUN_STEP && (!A.heun || (g & 1) == 0) && tid >= 32) {
-            const double t1 = time_of_step(A.t0, A.n0 + (A.heun ? (g >> 1) : g) + 1, A.dt);
+        if (MODE >= KM_EULER && (MODE != KM_HEUN || (g & 1) == 0) && tid >= 32) {
+            const double t1 = time_of_step(A.t0, A.n0 + (MODE == KM_HEUN ? (g >> 1) : g) + 1, A.dt);
             for (int sl = tid - 32; sl < nd; sl += NT - 32) Ls[sl] = stroke_length(t1, phs[sl], A.ell, A.lambda, A.omega);
         }
         if (stepping && A.n_cta > 1) __syncthreads();   // the barrier has been passed (thread 0)
@@ -418,7 +424,7 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
         DS_PROBE(11);
 
 
-        if (resident) {
+        if constexpr (RESIDENT) {
             // ---- resident stream: LDGSTS copies (generic proxy, L2 -> shared, 16 bytes per thread and piece) ----
             const uint4 *gsrc = reinterpret_cast<const uint4 *>(units);
             uint4 *sdst = reinterpret_cast<uint4 *>(smem_raw);
@@ -518,91 +524,91 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
         __syncthreads();  // every chunk consumed by every warp: the ring is free and becomes scratch
         DS_PROBE(4);
 
-        // ---- sum over the n_jg beta-groups (fixed order): red[jg][o] -> red2[part][o] ----
-        T *red = reinterpret_cast<T *>(smem_raw);   // [n_jg][n_out]   <= 12 NT
-        T *red2 = red + 12 * NT;                    // [nparts][n_out] <= 12 NT     (2 x 12 NT x 8 B = 96 KB = NS_MIN slots)
+        // ---- sum over the n_jg beta-groups (fixed order) ----
+        T *red = reinterpret_cast<T *>(smem_raw);   // [NT][12]  <= 48 KB
         if (active) {
-#pragma unroll
-            for (int k = 0; k < QI; ++k)
-#pragma unroll
-                for (int cc = 0; cc < 3; ++cc) red[red_w + (k * 3 + cc) * nq] = P::hsum(acc[k][cc]);
-        }
-        __syncthreads();
-        if (nparts > 1) {            // n_out * nparts <= NT: one (o, part) task per thread
-            if (l2_part < nparts) {
-                const T *rp = red + l2_o;
-                T sa = T(0), sb = T(0);
-                int gq = l2_part;
-                for (; gq + nparts < n_jg; gq += 2 * nparts) {
-                    sa += rp[gq * n_out];
-                    sb += rp[(gq + nparts) * n_out];
-                }
-                if (gq < n_jg) sa += rp[gq * n_out];
-                red2[l2_part * n_out + l2_o] = sa + sb;
-            }
-        } else {                     // one part: thread o sums all groups
-            for (int o = tid; o < n_out; o += NT) {
-                T sa = T(0), sb = T(0);
-                int gq = 0;
-                for (; gq + 1 < n_jg; gq += 2) {
-                    sa += red[gq * n_out + o];
-                    sb += red[(gq + 1) * n_out + o];
-                }
-                if (gq < n_jg) sa += red[gq * n_out + o];
-                red2[o] = sa + sb;
-            }
+            typename P::T4 *rw = reinterpret_cast<typename P::T4 *>(red + 12 * tid);
+            rw[0] = P::make4(P::hsum(acc[0][0]), P::hsum(acc[0][1]), P::hsum(acc[0][2]), P::hsum(acc[1][0]));
+            rw[1] = P::make4(P::hsum(acc[1][1]), P::hsum(acc[1][2]), P::hsum(acc[2][0]), P::hsum(acc[2][1]));
+            rw[2] = P::make4(P::hsum(acc[2][2]), P::hsum(acc[3][0]), P::hsum(acc[3][1]), P::hsum(acc[3][2]));
         }
         __syncthreads();
         DS_PROBE(5);
-        // u of state element e = 3 il + cc (local row il, component cc): the parts are added, then Eq. (3a)
-        // and the 1/(8 pi mu) factor in FP64
-        auto velocity = [&](int e, double Fi) {
-            const int il = e / 3, cc = e - 3 * il;
-            const T *rp = red2 + ((il & 3) * 3 + cc) * nq + (il >> 2);
-            T sum = rp[0];
-            for (int part = 1; part < nparts; ++part) sum += rp[part * n_out];
-            return A.self_mob * Fi + A.pre * (double)sum;
-        };
-
-        if (!stepping) {  // ---- RUN_APPLY: a2 + a3 with the stream's own F ----
-            for (int e = tid; e < 3 * nrows; e += NT) {
-                const long long i = r0 + e / 3;
-                reinterpret_cast<T *>(A.out_u)[(size_t)3 * r0 + e] = (T)velocity(e, (double)units[unit_index<T>(i, 3 + e % 3)]);
-            }
-        } else if (A.mode == RUN_VELOCITY) {
-            for (int e = tid; e < 3 * nrows; e += NT)
-                reinterpret_cast<T *>(A.out_u)[sys3 + (size_t)3 * r0 + e] = (T)velocity(e, Fs[e]);
-        } else {  // ---- RUN_STEP: integrator, one thread per state element ----
-            const bool pred = A.heun && (g & 1) == 0, corr = A.heun && (g & 1) == 1;
-            for (int e = tid; e < 3 * nrows; e += NT) {
-                const double v = velocity(e, Fs[e]);
-                double xn;
-                if (pred) {            // X* = X_n + dt V1
-                    V1s[e] = v;
-                    xn = Xs[e] + A.dt * v;
-                } else if (corr) {     // X_{n+1} = X_n + (dt/2)(V1 + V2)
-                    xn = Xs[e] + (0.5 * A.dt) * (V1s[e] + v);
-                    Xs[e] = xn;
-                } else {               // Euler
-                    xn = Xs[e] + A.dt * v;
-                    Xs[e] = xn;
+        if (tid < ((n_task * RP + 31) & ~31)) {        // the warps that hold tasks
+            const bool pred = MODE == KM_HEUN && (g & 1) == 0, corr = MODE == KM_HEUN && (g & 1) == 1;
+            for (int task = my_task; task < ((n_task + 3) & ~3); task += NT / RP) {   // warp-uniform trip count (4 tasks per warp)
+                T s0 = T(0), s1 = T(0), s2 = T(0), s3 = T(0);
+                if (task < n_task) {
+                    const int tq = task / 3, mq = task - 3 * tq;        // quad, which 4 of its 12 elements
+                    const typename P::T4 *rp = reinterpret_cast<const typename P::T4 *>(red + 12 * tq + 4 * mq);
+                    for (int gq = my_part; gq < n_jg; gq += RP) {
+                        const typename P::T4 v = rp[3 * nq * gq];
+                        s0 += v.x; s1 += v.y; s2 += v.z; s3 += v.w;
+                    }
                 }
-                Xc[e] = xn;
-                if (XcT != nullptr) XcT[e] = (T)xn;
+                DS_PROBE(18);
+#pragma unroll
+                for (int d = 1; d < RP; d <<= 1) {
+                    s0 += __shfl_xor_sync(0xffffffffu, s0, d); s1 += __shfl_xor_sync(0xffffffffu, s1, d);
+                    s2 += __shfl_xor_sync(0xffffffffu, s2, d); s3 += __shfl_xor_sync(0xffffffffu, s3, d);
+                }
+                DS_PROBE(19);
+                if (my_part != 0 || task >= n_task) continue;
+                // state elements e0 .. e0 + 3 of the CTA (e = 3 (local row) + component): Eq. (3a) and the
+                // 1/(8 pi mu) factor in FP64, then the integrator.  Straight-line: the four elements
+                // are independent and only the stores are predicated (the state arrays are padded to whole quads).
+                const int e0 = 4 * task;
+                const T sums[4] = {s0, s1, s2, s3};
+                if constexpr (!stepping) {               // RUN_APPLY: a2 + a3 with the stream's own F
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        const int e = e0 + j;
+                        if (e < 3 * nrows) {
+                            const double Fi = (double)units[unit_index<T>(r0 + e / 3, 3 + e % 3)];
+                            reinterpret_cast<T *>(A.out_u)[(size_t)3 * r0 + e] = (T)(A.self_mob * Fi + A.pre * (double)sums[j]);
+                        }
+                    }
+                } else {
+                double v[4], xo[4], v1[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) { v[j] = A.self_mob * Fs[e0 + j] + A.pre * (double)sums[j]; xo[j] = Xs[e0 + j]; v1[j] = V1s[e0 + j]; }
+                if (MODE == KM_VELOCITY) {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+                        if (e0 + j < 3 * nrows) reinterpret_cast<T *>(A.out_u)[sys3 + (size_t)3 * r0 + e0 + j] = (T)v[j];
+                    continue;
+                }
+                // predictor X* = X_n + dt V1;  corrector X_{n+1} = X_n + (dt/2)(V1 + V2);  Euler X_{n+1} = X_n + dt V
+                const double cdt = corr ? 0.5 * A.dt : A.dt;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int e = e0 + j;
+                    const double w = corr ? v1[j] + v[j] : v[j];
+                    const double xn = xo[j] + cdt * w;
+                    if (pred) V1s[e] = v[j]; else Xs[e] = xn;
+                    Xc[e] = xn;
+                    if (XcT != nullptr) XcT[e] = (T)xn;
+                }
+                }
             }
+        }
+        if (MODE >= KM_EULER) {
             __syncthreads();
+            DS_PROBE(17);
             // Eq. (4) at the new positions and time, one thread per dumbbell; publish the next stage's rows
-            T *un = reinterpret_cast<T *>(A.units[(A.cur + g + 1) & 1]) + (size_t)b * A.unit_stride * (6 * W);
-            for (int sl = tid; sl < nd; sl += NT) {
-                double x0[3], x1[3], F0[3];
+            if (tid < ((nd + 31) & ~31)) {
+                T *un = reinterpret_cast<T *>(A.units[(A.cur + g + 1) & 1]) + (size_t)b * A.unit_stride * (6 * W);
+                for (int sl = tid; sl < nd; sl += NT) {
+                    double x0[3], x1[3], F0[3];
 #pragma unroll
-                for (int cc = 0; cc < 3; ++cc) { x0[cc] = Xc[6 * sl + cc]; x1[cc] = Xc[6 * sl + 3 + cc]; }
-                dumbbell_force(x0, x1, Ls[sl], A.k0, F0);
+                    for (int cc = 0; cc < 3; ++cc) { x0[cc] = Xc[6 * sl + cc]; x1[cc] = Xc[6 * sl + 3 + cc]; }
+                    dumbbell_force(x0, x1, Ls[sl], A.k0, F0);
 #pragma unroll
-                for (int cc = 0; cc < 3; ++cc) { Fs[6 * sl + cc] = F0[cc]; Fs[6 * sl + 3 + cc] = -F0[cc]; }
-                if (g + 1 < n_stage) publish_dumbbell(un, r0 + 2 * sl, x0, x1, F0);
+                    for (int cc = 0; cc < 3; ++cc) { Fs[6 * sl + cc] = F0[cc]; Fs[6 * sl + 3 + cc] = -F0[cc]; }
+                    if (g + 1 < n_stage) publish_dumbbell(un, r0 + 2 * sl, x0, x1, F0);
+                }
+                fence_proxy_async_global();   // the stream is also read through the async proxy (TMA)
             }
-            fence_proxy_async_global();   // the stream is also read through the async proxy (TMA)
         }
         DS_PROBE(6);
         fence_proxy_async_shared();
@@ -610,7 +616,7 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
         DS_PROBE(7);
     }
 
-    if (A.mode == RUN_STEP && A.state_smem)
+    if (MODE >= KM_EULER && A.state_smem)
         for (int e = tid; e < 3 * nrows; e += NT) A.X[sys3 + 3 * r0 + e] = Xs[e];
 }
 

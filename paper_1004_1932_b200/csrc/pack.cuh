@@ -18,6 +18,7 @@ template <> struct Pack<float> {
     typedef float4 T4;
     static constexpr int W = 2;  // j-spheres per pack
     static __device__ __forceinline__ V bc(float s) { return make_float2(s, s); }
+    static __device__ __forceinline__ T4 make4(float a, float b, float c, float d) { return make_float4(a, b, c, d); }
     static __device__ __forceinline__ V sub(V a, V b) {
         // sub.f32x2 -> FADD2 with a negated source modifier (no extra instruction)
         unsigned long long r;
@@ -49,6 +50,7 @@ template <> struct Pack<double> {
     typedef double4 T4;
     static constexpr int W = 1;
     static __device__ __forceinline__ V bc(double s) { return s; }
+    static __device__ __forceinline__ T4 make4(double a, double b, double c, double d) { return make_double4(a, b, c, d); }
     static __device__ __forceinline__ V sub(V a, V b) { return a - b; }
     static __device__ __forceinline__ V mul(V a, V b) { return a * b; }
     static __device__ __forceinline__ V fma(V a, V b, V c) { return ::fma(a, b, c); }
