@@ -3,6 +3,7 @@
 // No arithmetic of the method lives here; it is all in mobility.cuh / state.cuh.
 #include <cuda_runtime.h>
 #include <math.h>
+#include <stdint.h>
 #include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
@@ -537,26 +538,35 @@ int ds_mobility_apply(ds_system *s, const void *pos, const void *F, void *u, int
     if (!dF_dev) { DS_TRY(ensure(s->st_b, nb)); CU_TRY(cudaMemcpyAsync(s->st_b.p, F, nb, cudaMemcpyHostToDevice, s->stream)); dF = s->st_b.p; }
     if (!du_dev) { DS_TRY(ensure(s->st_c, nb)); du = s->st_c.p; }
 
-    // user arrays -> one beta-stream (pack kernel), then the mobility kernel in RUN_APPLY mode
+    // the mobility kernel in RUN_APPLY mode.  A stream that fits one CTA's shared memory is packed by every CTA
+    // for itself, straight from the user's arrays; a larger one goes through the pack kernel and a global stream.
     const int U = (n + s->W - 1) / s->W;
-    const long long n_units = (long long)U + ds::PAD_UNITS;
-    DS_TRY(ensure(s->ap_units, (size_t)n_units * ds::UNIT_BYTES));
-    const unsigned pg = (unsigned)((n_units + 255) / 256);
-    if (f64)
-        ds::pack_user_kernel<double><<<pg, 256, 0, s->stream>>>((const double *)dpos, (const double *)dF, (double *)s->ap_units.p, n, n_units);
-    else
-        ds::pack_user_kernel<float><<<pg, 256, 0, s->stream>>>((const float *)dpos, (const float *)dF, (float *)s->ap_units.p, n, n_units);
-    CU_TRY(cudaGetLastError());
-    s->launches += 1;
     ds::RunArgs A;
     memset(&A, 0, sizeof A);
-    A.N = n; A.NQ = (n + ds::QI - 1) / ds::QI; A.U = U; A.unit_stride = n_units;
+    A.N = n; A.NQ = (n + ds::QI - 1) / ds::QI; A.U = U;
     A.n_cta = choose_tiles_apply(s, A.NQ, A.U);
     A.buf_bytes = (ds::SMEM_MAX - ds::BAR_BYTES) / 128 * 128;
     fill_constants(s, A);
     A.mode = ds::RUN_APPLY;
-    A.units[0] = s->ap_units.p; A.units[1] = s->ap_units.p; A.out_u = du;
+    A.out_u = du;
     A.probe = s->probe;
+    const bool aligned = (((uintptr_t)dpos | (uintptr_t)dF) & 7u) == 0;   // the in-kernel pack reads 8-byte pairs
+    if (aligned && stream_resident(A.NQ, A.U, A.n_cta, A.buf_bytes)) {
+        A.raw_pos = dpos; A.raw_F = dF;
+        A.unit_stride = (long long)U + ds::PAD_UNITS;
+    } else {
+        const long long n_units = (long long)U + ds::PAD_UNITS;
+        DS_TRY(ensure(s->ap_units, (size_t)n_units * ds::UNIT_BYTES));
+        const unsigned pg = (unsigned)((n_units + 255) / 256);
+        if (f64)
+            ds::pack_user_kernel<double><<<pg, 256, 0, s->stream>>>((const double *)dpos, (const double *)dF, (double *)s->ap_units.p, n, n_units);
+        else
+            ds::pack_user_kernel<float><<<pg, 256, 0, s->stream>>>((const float *)dpos, (const float *)dF, (float *)s->ap_units.p, n, n_units);
+        CU_TRY(cudaGetLastError());
+        s->launches += 1;
+        A.unit_stride = n_units;
+        A.units[0] = s->ap_units.p; A.units[1] = s->ap_units.p;
+    }
     DS_TRY(launch_run(s, A, dim3((unsigned)A.n_cta, 1), (size_t)A.buf_bytes + ds::BAR_BYTES, false, s->stream));
     if (!du_dev) {
         CU_TRY(cudaMemcpyAsync(u, du, nb, cudaMemcpyDeviceToHost, s->stream));

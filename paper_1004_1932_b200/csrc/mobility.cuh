@@ -35,6 +35,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <type_traits>
+
 #include "pack.cuh"
 
 namespace ds {
@@ -51,7 +53,7 @@ constexpr int CHU = 512;                 // units per ring slot (24 KB)
 constexpr int SLOT_BYTES = CHU * UNIT_BYTES;
 constexpr int NS_MAX = 8;                // ring slots (192 KB)
 constexpr int NS_MIN = 4;                // the reduction scratch aliases the first 4 slots (96 KB)
-constexpr int BAR_BYTES = (2 * NS_MAX + 4) * 8;
+constexpr int BAR_BYTES = 512;           // mbarriers (2 NS_MAX + 3) and the resident mode's segment table (8 x 16 B)
 constexpr int SMEM_MAX = 232448;         // 227 KB opt-in limit per CTA on sm_100
 constexpr int PAD_UNITS = CHU;           // dummy units appended to every system's stream
 constexpr int STATE_BYTES_PER_ROW = 15 * 8 + 8;  // X_n, X of the stage (FP64 and rounded to T), V1, F (3 x 8 B each) + (phase, L) per dumbbell = 16 B / 2 rows
@@ -75,6 +77,7 @@ struct RunArgs {
     int heun;                 // RUN_STEP: 1 = Heun (2 stages per step), 0 = Euler
     long long n0, n_steps;    // RUN_STEP: index of the first step, number of steps
     void *out_u;              // RUN_APPLY / RUN_VELOCITY: u [B][N][3] user precision
+    const void *raw_pos, *raw_F;  // RUN_APPLY with a resident stream: the user's [n][3] arrays (each CTA packs them itself)
     double *X;                // state positions [B][N][3] (read at start; written at the end of RUN_STEP)
     const double *phase;      // [B][S]
     double t0, dt, ell, lambda, omega, k0;
@@ -192,7 +195,7 @@ __device__ __forceinline__ void pair_unit(const V2<T> *__restrict__ p, const typ
 // Eq. (4).  Explicit rounding (no contraction) so that every call site produces
 // the same bits for the same inputs: ds_step(n) is bit-identical however the n steps are split.
 //   L^s(t) = ell + lambda sin(omega t + phi^s)
-__device__ __forceinline__ double stroke_length(double t, double phi, double ell, double lambda, double omega) {
+__device__ __noinline__ double stroke_length(double t, double phi, double ell, double lambda, double omega) {
     return __dadd_rn(ell, __dmul_rn(lambda, sin(__dadd_rn(__dmul_rn(omega, t), phi))));
 }
 //   n = (X_{2s+1} - X_{2s})/d, g = k0 (d - L), F_{2s} = +g n, F_{2s+1} = -g n   (F = -dU/dX)
@@ -241,6 +244,37 @@ __device__ __forceinline__ void publish_dumbbell(double *un, long long i0, const
     p[5] = make_double2(-F0[1], -F0[2]);
 }
 
+
+// Unit u of the stream built from the user's arrays pos, F [n][3] (RUN_APPLY): spheres beyond n are far-away
+// zero-force dummies.  FP32: spheres 2u, 2u + 1 -> [x0 x1][y0 y1][z0 z1][fx0 fx1][fy0 fy1][fz0 fz1]; FP64: sphere u.
+__device__ __forceinline__ void pack_unit(float4 *dst, const float *pos, const float *F, int u, int n) {
+    const float D = Pack<float>::dummy();
+    float a[6] = {D, D, D, D, D, D}, f[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    if (2 * u + 1 < n) {
+        const float2 *pp = reinterpret_cast<const float2 *>(pos + 6 * (size_t)u), *fp = reinterpret_cast<const float2 *>(F + 6 * (size_t)u);
+        const float2 p0 = __ldg(pp), p1 = __ldg(pp + 1), p2 = __ldg(pp + 2), f0 = __ldg(fp), f1 = __ldg(fp + 1), f2 = __ldg(fp + 2);
+        a[0] = p0.x; a[1] = p0.y; a[2] = p1.x; a[3] = p1.y; a[4] = p2.x; a[5] = p2.y;
+        f[0] = f0.x; f[1] = f0.y; f[2] = f1.x; f[3] = f1.y; f[4] = f2.x; f[5] = f2.y;
+    } else if (2 * u < n) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { a[c] = __ldg(pos + 6 * (size_t)u + c); f[c] = __ldg(F + 6 * (size_t)u + c); }
+    }
+    dst[0] = make_float4(a[0], a[3], a[1], a[4]);
+    dst[1] = make_float4(a[2], a[5], f[0], f[3]);
+    dst[2] = make_float4(f[1], f[4], f[2], f[5]);
+}
+__device__ __forceinline__ void pack_unit(double2 *dst, const double *pos, const double *F, int u, int n) {
+    const double D = Pack<double>::dummy();
+    double a[3] = {D, D, D}, f[3] = {0.0, 0.0, 0.0};
+    if (u < n) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { a[c] = __ldg(pos + 3 * (size_t)u + c); f[c] = __ldg(F + 3 * (size_t)u + c); }
+    }
+    dst[0] = make_double2(a[0], a[1]);
+    dst[1] = make_double2(a[2], f[0]);
+    dst[2] = make_double2(f[1], f[2]);
+}
+
 #ifdef DS_ENABLE_PROBE
 #define DS_PROBE(slot)                                                                          \
     do {                                                                                        \
@@ -263,6 +297,7 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
     uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + buf_bytes);
     uint64_t *empty = full + NS_MAX;
     uint64_t *gran = empty + NS_MAX;     // resident mode: one barrier per granule of the stream (3)
+    int4 *segs = reinterpret_cast<int4 *>(gran + 4);   // resident mode: the stage's tight loops (<= 8), see below
 
     const int tid = threadIdx.x, lane = tid & 31;
     const int c = blockIdx.x, b = A.b0 + blockIdx.y;
@@ -340,6 +375,22 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
         mbar_init(gran + 1, 1);    // G1, G2: thread 0's TMA bulk copies
         mbar_init(gran + 2, 1);
         mbar_fence_init();
+        if (RESIDENT) {
+            // a new tight loop starts where a granule begins, where the guard ends and where the stream wraps around
+            const int wrapq = total_it - it_own;
+            int q = 0, n = 0;
+            while (q < total_it) {
+                int qe = q < h0 ? h0 : (q < h0 + h1 ? h0 + h1 : total_it);
+                if (q < n_guard && n_guard < qe) qe = n_guard;
+                if (q < wrapq && wrapq < qe) qe = wrapq;
+                int it = it_own + q;
+                it = it >= total_it ? it - total_it : it;
+                const int w = (q == h0 && h1 > 0) ? 1 : ((q == h0 + h1 && h2 > 0) ? 2 : -1);
+                segs[n++] = make_int4(it * stride, qe - q, w, q < n_guard ? it + 1 : 0);
+                q = qe;
+            }
+            segs[7].x = n;
+        }
     }
 
     const int n_stage = MODE >= KM_EULER ? (int)(A.n_steps * (MODE == KM_HEUN ? 2 : 1)) : 1;
@@ -413,9 +464,14 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
                 if (XcT != nullptr && stepping) {
                     x = XcT[3 * il]; y = XcT[3 * il + 1]; z = XcT[3 * il + 2];
                 } else {
-                    x = __ldcg(units + unit_index<T>(r0 + il, 0));
-                    y = __ldcg(units + unit_index<T>(r0 + il, 1));
-                    z = __ldcg(units + unit_index<T>(r0 + il, 2));
+                    if (MODE == KM_APPLY && A.raw_pos != nullptr) {
+                        const T *rp = reinterpret_cast<const T *>(A.raw_pos) + 3 * (r0 + il);
+                        x = __ldg(rp); y = __ldg(rp + 1); z = __ldg(rp + 2);
+                    } else {
+                        x = __ldcg(units + unit_index<T>(r0 + il, 0));
+                        y = __ldcg(units + unit_index<T>(r0 + il, 1));
+                        z = __ldcg(units + unit_index<T>(r0 + il, 2));
+                    }
                 }
             }
             xi[k][0] = P::bc(x); xi[k][1] = P::bc(y); xi[k][2] = P::bc(z);
@@ -434,43 +490,54 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
                 cp_async16(sdst + a, gsrc + a);
             };
             const uint32_t par = (uint32_t)g & 1u;  // every granule barrier completes one phase per stage
-            if (tid == 0) {   // G1, G2: TMA bulk copies of consumption pieces [j0, j1) (two copies where the range wraps)
-                auto tma_range = [&](int j0, int j1, uint64_t *bar) {
-                    int a0 = sp + j0;
-                    a0 = a0 >= tp ? a0 - tp : a0;
-                    const int len = j1 - j0, first = a0 + len <= tp ? len : tp - a0;
-                    mbar_expect_tx(bar, (uint32_t)len * 16u);
-                    bulk_g2s(sdst + a0, gsrc + a0, (uint32_t)first * 16u, bar);
-                    if (first < len) bulk_g2s(sdst, gsrc, (uint32_t)(len - first) * 16u, bar);
-                };
-                if (h1 > 0) tma_range(pA, pAB, gran + 1);
-                if (h2 > 0) tma_range(pAB, tp, gran + 2);
+            if (MODE == KM_APPLY && A.raw_pos != nullptr) {
+                // stateless apply: the CTA packs the user's arrays into its resident stream itself (no pack kernel,
+                // no global intermediate); CTAs start at different units so that they do not read L2 in a convoy
+                typedef typename std::conditional<sizeof(T) == 4, float4, double2>::type Q;
+                const int up = total_it * n_jg;
+                int u = tid + (int)(((long long)c * up) / A.n_cta);
+                for (int k = tid; k < up; k += NT, u += NT) {
+                    u = u >= up ? u - up : u;
+                    pack_unit(reinterpret_cast<Q *>(smem_raw) + 3 * u, reinterpret_cast<const T *>(A.raw_pos),
+                              reinterpret_cast<const T *>(A.raw_F), u, A.N);
+                }
+                __syncthreads();
+                mbar_arrive(gran + 0);
+                if (tid == 0) { mbar_arrive(gran + 1); mbar_arrive(gran + 2); }
+            } else {
+                if (tid == 0) {   // G1, G2: TMA bulk copies of consumption pieces [j0, j1) (two copies where the range wraps)
+                    auto tma_range = [&](int j0, int j1, uint64_t *bar) {
+                        int a0 = sp + j0;
+                        a0 = a0 >= tp ? a0 - tp : a0;
+                        const int len = j1 - j0, first = a0 + len <= tp ? len : tp - a0;
+                        mbar_expect_tx(bar, (uint32_t)len * 16u);
+                        bulk_g2s(sdst + a0, gsrc + a0, (uint32_t)first * 16u, bar);
+                        if (first < len) bulk_g2s(sdst, gsrc, (uint32_t)(len - first) * 16u, bar);
+                    };
+                    if (h1 > 0) tma_range(pA, pAB, gran + 1);
+                    if (h2 > 0) tma_range(pAB, tp, gran + 2);
+                }
+                for (int j = tid; j < pA; j += NT) copy_piece(j);   // G0: LDGSTS by every thread (lowest latency)
+                cp_async_arrive(gran + 0);
             }
-            for (int j = tid; j < pA; j += NT) copy_piece(j);   // G0: LDGSTS by every thread (lowest latency)
-            cp_async_arrive(gran + 0);
             DS_PROBE(10);
             const V2<T> *const base = reinterpret_cast<const V2<T> *>(smem_raw) + 3 * jg;
             mbar_wait(gran + 0, par);
             DS_PROBE(2);
-            // the stage's total_it iterations (each: QI alpha x 1 unit per thread) as a few tight loops: a new one
-            // starts where a granule begins, where the guard ends and where the stream wraps around
-            const int wrapq = total_it - it_own;
-            int q = 0;
-            while (q < total_it) {
-                if (q == h0 && h1 > 0) { DS_PROBE(13); mbar_wait(gran + 1, par); DS_PROBE(14); }
-                if (q == h0 + h1 && h2 > 0) { DS_PROBE(15); mbar_wait(gran + 2, par); DS_PROBE(16); }
-                int qe = q < h0 ? h0 : (q < h0 + h1 ? h0 + h1 : total_it);
-                if (q < n_guard && n_guard < qe) qe = n_guard;
-                if (q < wrapq && wrapq < qe) qe = wrapq;
-                int it = it_own + q;
-                it = it >= total_it ? it - total_it : it;
-                const V2<T> *p = base + it * stride;
-                if (q < n_guard) {
+            const int nseg = segs[7].x;
+            // the stage's total_it iterations (each: QI alpha x 1 unit per thread) as the few tight loops of the
+            // segment table (built once, stage-invariant): {first piece, iterations, granule to wait for or -1,
+            // first iteration + 1 if the segment holds own rows else 0}
+            for (int sgi = 0; sgi < nseg; ++sgi) {
+                const int4 sg = segs[sgi];
+                if (sg.z >= 0) mbar_wait(gran + sg.z, par);
+                const V2<T> *p = base + sg.x;
+                if (sg.w != 0) {
                     // iterations that hold the CTA's own rows: a warp takes the guarded variant (r = 0 excluded)
                     // only if one of its lanes reads an own unit in that iteration
-                    int u = it * n_jg + jg;
+                    int u = (sg.w - 1) * n_jg + jg;
 #pragma unroll 1
-                    for (int r = q; r < qe; ++r, p += stride, u += n_jg) {
+                    for (int r = 0; r < sg.y; ++r, p += stride, u += n_jg) {
                         const bool own = __any_sync(0xffffffffu, active && u >= d0 && u < d1);
                         if (active) {
                             if (own) pair_unit<T, TENSOR, true>(p, xi, acc, c1, negc2);
@@ -478,10 +545,9 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
                         }
                     }
                 } else if (active) {
-#pragma unroll 2
-                    for (int r = q; r < qe; ++r, p += stride) pair_unit<T, TENSOR, false>(p, xi, acc, c1, negc2);
+#pragma unroll 1
+                    for (int r = 0; r < sg.y; ++r, p += stride) pair_unit<T, TENSOR, false>(p, xi, acc, c1, negc2);
                 }
-                q = qe;
             }
         } else {
             // ---- ring of slots filled by TMA bulk copies (thread 0), one tight loop per chunk ----
@@ -564,7 +630,8 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
                     for (int j = 0; j < 4; ++j) {
                         const int e = e0 + j;
                         if (e < 3 * nrows) {
-                            const double Fi = (double)units[unit_index<T>(r0 + e / 3, 3 + e % 3)];
+                            const double Fi = A.raw_F != nullptr ? (double)reinterpret_cast<const T *>(A.raw_F)[(size_t)3 * r0 + e]
+                                                                 : (double)units[unit_index<T>(r0 + e / 3, 3 + e % 3)];
                             reinterpret_cast<T *>(A.out_u)[(size_t)3 * r0 + e] = (T)(A.self_mob * Fi + A.pre * (double)sums[j]);
                         }
                     }
