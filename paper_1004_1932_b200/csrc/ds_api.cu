@@ -70,6 +70,8 @@ struct ds_system {
     void *units[2] = {nullptr, nullptr};        // beta-streams (mobility.cuh), ping-pong over the stages
     unsigned long long *bar = nullptr;          // [B] arrival counters of the inter-CTA barrier
     unsigned long long bar_base = 0;
+    void *ll[2] = {nullptr, nullptr};           // tagged (low-latency) copies of the streams, 96 B per unit
+    unsigned int ll_tag = 1;                    // next unused tag (0 = never written)
     double *Xcg = nullptr, *V1g = nullptr, *Fg = nullptr, *Lg = nullptr;  // only when !state_smem
     long long *probe = nullptr;                 // caller's device buffer (ds_set_probe) or NULL
     // scratch of the stateless apply and of host-pointer staging
@@ -250,15 +252,29 @@ int launch_state_run(ds_system *s, int mode, long long n_steps, void *out_u) {
     A.n0 = s->n_host; A.n_steps = n_steps; A.out_u = out_u;
     A.X = s->X; A.phase = s->phase;
     A.bar = s->bar; A.bar_base = s->bar_base;
+    // low-latency stage hand-over (tagged stream copy) pays off when many CTAs meet at the barrier (measured: 147 CTAs
+    // -9 % per stage, 2 CTAs +5 %)
+    const bool low_latency = s->n_cta > 16;
+    A.ll[0] = low_latency ? s->ll[0] : nullptr; A.ll[1] = low_latency ? s->ll[1] : nullptr;
+    A.h0_ll = 4;
     A.state_smem = s->state_smem; A.Xcg = s->Xcg; A.V1g = s->V1g; A.Fg = s->Fg; A.Lg = s->Lg;
     A.probe = s->probe;
     const long long n_stage = mode == ds::RUN_STEP ? n_steps * (A.heun ? 2 : 1) : 1;
+    // tags ll_tag .. ll_tag + n_stage are used by this call; a tag value is never reused while it may still sit in
+    // a buffer: on wrap-around of the 32-bit counter the buffers are cleared
+    if ((unsigned long long)s->ll_tag + (unsigned long long)n_stage + 1ULL >= 0xffffffffULL) {
+        const size_t ub = (size_t)s->B * (size_t)s->unit_stride * ds::UNIT_BYTES;
+        for (int k = 0; k < 2; ++k) CU_TRY(cudaMemsetAsync(s->ll[k], 0, 2 * ub, s->stream));
+        s->ll_tag = 1;
+    }
+    A.ll_tag0 = s->ll_tag;
     for (int b0 = 0; b0 < s->B; b0 += s->sys_per_launch) {
         const int nb = s->B - b0 < s->sys_per_launch ? s->B - b0 : s->sys_per_launch;
         A.b0 = b0;
         DS_TRY(launch_run(s, A, dim3((unsigned)s->n_cta, (unsigned)nb), s->smem_bytes, s->n_cta > 1, s->stream));
     }
     if (s->n_cta > 1) s->bar_base += (unsigned long long)s->n_cta * (unsigned long long)n_stage;
+    s->ll_tag += (unsigned int)n_stage + 1u;
     return DS_OK;
 }
 
@@ -393,12 +409,15 @@ int ds_create(const ds_params *p, ds_system **out) {
     al((void **)&s->X, n3 * 8);
     al((void **)&s->phase, (size_t)s->B * s->S * 8);
     al(&s->units[0], ub); al(&s->units[1], ub);
+    al(&s->ll[0], 2 * ub); al(&s->ll[1], 2 * ub);
     al((void **)&s->bar, (size_t)s->B * sizeof(unsigned long long));
     // global homes of the per-row state, used only by tiles too large for shared memory (any tuning)
     al((void **)&s->Xcg, n3 * 8); al((void **)&s->V1g, n3 * 8); al((void **)&s->Fg, n3 * 8);
     al((void **)&s->Lg, (size_t)s->B * s->S * 8);
     if (e != cudaSuccess) { snprintf(g_cuda_err, sizeof g_cuda_err, "cudaMalloc -> %s", cudaGetErrorString(e)); (void)cudaGetLastError(); return fail(DS_ERR_ALLOC); }
     if (cudaMemsetAsync(s->bar, 0, (size_t)s->B * sizeof(unsigned long long), s->stream) != cudaSuccess) return fail(DS_ERR_CUDA);
+    for (int k = 0; k < 2; ++k)
+        if (cudaMemsetAsync(s->ll[k], 0, 2 * ub, s->stream) != cudaSuccess) return fail(DS_ERR_CUDA);
     for (int k = 0; k < 2 && rc == DS_OK; ++k) rc = f64 ? run_pad_init<double>(s, s->units[k]) : run_pad_init<float>(s, s->units[k]);
     if (rc != DS_OK) return fail(rc);
     if (cudaStreamSynchronize(s->stream) != cudaSuccess) return fail(DS_ERR_CUDA);
@@ -410,7 +429,7 @@ int ds_destroy(ds_system *s) {
     if (!s) return DS_OK;
     cudaSetDevice(s->P.device);
     cudaStreamSynchronize(s->stream);
-    void *ptrs[] = {s->X, s->phase, s->units[0], s->units[1], s->bar, s->Xcg, s->V1g, s->Fg, s->Lg,
+    void *ptrs[] = {s->X, s->phase, s->units[0], s->units[1], s->ll[0], s->ll[1], s->bar, s->Xcg, s->V1g, s->Fg, s->Lg,
                     s->ap_units.p, s->st_a.p, s->st_b.p, s->st_c.p};
     for (void *q : ptrs) if (q) cudaFree(q);
     (void)cudaGetLastError();

@@ -53,7 +53,7 @@ constexpr int CHU = 512;                 // units per ring slot (24 KB)
 constexpr int SLOT_BYTES = CHU * UNIT_BYTES;
 constexpr int NS_MAX = 8;                // ring slots (192 KB)
 constexpr int NS_MIN = 4;                // the reduction scratch aliases the first 4 slots (96 KB)
-constexpr int BAR_BYTES = 512;           // mbarriers (2 NS_MAX + 3) and the resident mode's segment table (8 x 16 B)
+constexpr int BAR_BYTES = 512;           // mbarriers (2 NS_MAX + 3) and the resident mode's segment table (12 x 16 B)
 constexpr int SMEM_MAX = 232448;         // 227 KB opt-in limit per CTA on sm_100
 constexpr int PAD_UNITS = CHU;           // dummy units appended to every system's stream
 constexpr int STATE_BYTES_PER_ROW = 15 * 8 + 8;  // X_n, X of the stage (FP64 and rounded to T), V1, F (3 x 8 B each) + (phase, L) per dumbbell = 16 B / 2 rows
@@ -84,6 +84,11 @@ struct RunArgs {
     // inter-CTA barrier: one monotonic arrival counter per system; this launch starts at bar_base
     unsigned long long *bar;
     unsigned long long bar_base;
+    // low-latency copy of the streams: every 32-bit word of a unit paired with a stage tag ({w0, tag, w1, tag} per
+    // 16 bytes, 96 B per unit); a reader that sees the tag has the word (8-byte accesses are single-copy atomic)
+    void *ll[2];
+    int h0_ll;                // iterations of the first granule in low-latency mode
+    unsigned int ll_tag0;     // tag of the stream the prologue publishes; stage g's output carries ll_tag0 + g + 1
     // state rows in shared memory (1) or, for very large tiles, in these global arrays (0)
     int state_smem;
     double *Xcg, *V1g, *Fg, *Lg;  // [B][N][3] x 3, [B][S]
@@ -225,25 +230,49 @@ template <typename T> __device__ __forceinline__ size_t unit_index(long long i, 
     return (size_t)(i / W) * (6 * W) + (size_t)c * W + (size_t)(i % W);
 }
 
-// The two spheres i0 (even), i0 + 1 of one dumbbell -> their units of a stream, rounded to T.
-__device__ __forceinline__ void publish_dumbbell(float *un, long long i0, const double (&x0)[3], const double (&x1)[3],
-                                                 const double (&F0)[3]) {
-    float4 *p = reinterpret_cast<float4 *>(un + (size_t)(i0 >> 1) * 12);  // one unit: [x0 x1][y0 y1][z0 z1][fx..][fy..][fz..]
-    p[0] = make_float4((float)x0[0], (float)x1[0], (float)x0[1], (float)x1[1]);
-    p[1] = make_float4((float)x0[2], (float)x1[2], (float)F0[0], (float)(-F0[0]));
-    p[2] = make_float4((float)F0[1], (float)(-F0[1]), (float)F0[2], (float)(-F0[2]));
+__device__ __forceinline__ uint4 ld_volatile_v4(const uint4 *p) {
+    uint4 v;
+    asm volatile("ld.volatile.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
+    return v;
 }
-__device__ __forceinline__ void publish_dumbbell(double *un, long long i0, const double (&x0)[3], const double (&x1)[3],
-                                                 const double (&F0)[3]) {
-    double2 *p = reinterpret_cast<double2 *>(un + (size_t)i0 * 6);  // two units of one sphere each: [x y z fx fy fz]
-    p[0] = make_double2(x0[0], x0[1]);
-    p[1] = make_double2(x0[2], F0[0]);
-    p[2] = make_double2(F0[1], F0[2]);
-    p[3] = make_double2(x1[0], x1[1]);
-    p[4] = make_double2(x1[2], -F0[0]);
-    p[5] = make_double2(-F0[1], -F0[2]);
+// the 16-byte piece (w0 w1 w2 w3) of a unit -> its two tagged quads
+__device__ __forceinline__ void publish_ll_piece(uint4 *q, uint32_t w0, uint32_t w1, uint32_t w2, uint32_t w3, uint32_t tag) {
+    q[0] = make_uint4(w0, tag, w1, tag);
+    q[1] = make_uint4(w2, tag, w3, tag);
+}
+__device__ __forceinline__ void publish_ll(uint4 *ll_units, long long i0, const float4 (&u)[3], uint32_t tag) {
+    uint4 *q = ll_units + (size_t)(i0 >> 1) * 6;       // FP32: one unit per dumbbell
+#pragma unroll
+    for (int k = 0; k < 3; ++k)
+        publish_ll_piece(q + 2 * k, __float_as_uint(u[k].x), __float_as_uint(u[k].y), __float_as_uint(u[k].z), __float_as_uint(u[k].w), tag);
+}
+__device__ __forceinline__ void publish_ll(uint4 *ll_units, long long i0, const double2 (&u)[6], uint32_t tag) {
+    uint4 *q = ll_units + (size_t)i0 * 6;              // FP64: two units (one sphere each) per dumbbell
+#pragma unroll
+    for (int k = 0; k < 6; ++k)
+        publish_ll_piece(q + 2 * k, (uint32_t)__double2loint(u[k].x), (uint32_t)__double2hiint(u[k].x),
+                         (uint32_t)__double2loint(u[k].y), (uint32_t)__double2hiint(u[k].y), tag);
 }
 
+// The two spheres i0 (even), i0 + 1 of one dumbbell -> their units of a stream, rounded to T.
+__device__ __forceinline__ void publish_dumbbell(float *un, uint4 *ll_units, uint32_t tag, long long i0, const double (&x0)[3],
+                                                 const double (&x1)[3], const double (&F0)[3]) {
+    float4 *p = reinterpret_cast<float4 *>(un + (size_t)(i0 >> 1) * 12);  // one unit: [x0 x1][y0 y1][z0 z1][fx..][fy..][fz..]
+    const float4 u[3] = {make_float4((float)x0[0], (float)x1[0], (float)x0[1], (float)x1[1]),
+                         make_float4((float)x0[2], (float)x1[2], (float)F0[0], (float)(-F0[0])),
+                         make_float4((float)F0[1], (float)(-F0[1]), (float)F0[2], (float)(-F0[2]))};
+    p[0] = u[0]; p[1] = u[1]; p[2] = u[2];
+    if (ll_units != nullptr) publish_ll(ll_units, i0, u, tag);
+}
+__device__ __forceinline__ void publish_dumbbell(double *un, uint4 *ll_units, uint32_t tag, long long i0, const double (&x0)[3],
+                                                 const double (&x1)[3], const double (&F0)[3]) {
+    double2 *p = reinterpret_cast<double2 *>(un + (size_t)i0 * 6);  // two units of one sphere each: [x y z fx fy fz]
+    const double2 u[6] = {make_double2(x0[0], x0[1]), make_double2(x0[2], F0[0]), make_double2(F0[1], F0[2]),
+                          make_double2(x1[0], x1[1]), make_double2(x1[2], -F0[0]), make_double2(-F0[1], -F0[2])};
+#pragma unroll
+    for (int k = 0; k < 6; ++k) p[k] = u[k];
+    if (ll_units != nullptr) publish_ll(ll_units, i0, u, tag);
+}
 
 // Unit u of the stream built from the user's arrays pos, F [n][3] (RUN_APPLY): spheres beyond n are far-away
 // zero-force dummies.  FP32: spheres 2u, 2u + 1 -> [x0 x1][y0 y1][z0 z1][fx0 fx1][fy0 fy1][fz0 fz1]; FP64: sphere u.
@@ -273,6 +302,18 @@ __device__ __forceinline__ void pack_unit(double2 *dst, const double *pos, const
     dst[0] = make_double2(a[0], a[1]);
     dst[1] = make_double2(a[2], f[0]);
     dst[2] = make_double2(f[1], f[2]);
+}
+
+// 16-byte piece p (0..2) of a far-away zero-force pad unit, as raw words
+template <typename T> __device__ __forceinline__ uint4 pad_piece(int p);
+template <> __device__ __forceinline__ uint4 pad_piece<float>(int p) {
+    const uint32_t D = __float_as_uint(Pack<float>::dummy());
+    return p == 0 ? make_uint4(D, D, D, D) : (p == 1 ? make_uint4(D, D, 0u, 0u) : make_uint4(0u, 0u, 0u, 0u));
+}
+template <> __device__ __forceinline__ uint4 pad_piece<double>(int p) {
+    const double Dd = Pack<double>::dummy();
+    const uint32_t lo = (uint32_t)__double2loint(Dd), hi = (uint32_t)__double2hiint(Dd);
+    return p == 0 ? make_uint4(lo, hi, lo, hi) : (p == 1 ? make_uint4(lo, hi, 0u, 0u) : make_uint4(0u, 0u, 0u, 0u));
 }
 
 #ifdef DS_ENABLE_PROBE
@@ -346,7 +387,8 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
     const int it_own = d0 / n_jg;
     const int n_guard = (d1 - 1) / n_jg - it_own + 1;
     const int sp = it_own * stride;                            // first piece in consumption order
-    const int h0 = total_it < 4 ? total_it : 4;
+    const int h0w = (RESIDENT && MODE != KM_APPLY && A.n_cta > 1 && A.ll[0] != nullptr) ? A.h0_ll : 4;  // low-latency mode: G0 also covers the barrier
+    const int h0 = total_it < h0w ? total_it : h0w;
     const int h1 = total_it - h0 < 6 ? total_it - h0 : 6;
     const int h2 = total_it - h0 - h1;
     const int pA = h0 * stride, pAB = (h0 + h1) * stride;      // piece index (consumption order) where G1 / G2 start
@@ -383,17 +425,23 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
                 int qe = q < h0 ? h0 : (q < h0 + h1 ? h0 + h1 : total_it);
                 if (q < n_guard && n_guard < qe) qe = n_guard;
                 if (q < wrapq && wrapq < qe) qe = wrapq;
+                if (h0w > 6 && q < h0 && q >= n_guard && q + 4 < qe) qe = q + 4;   // low-latency mode: thread 0 looks at the barrier between segments
                 int it = it_own + q;
                 it = it >= total_it ? it - total_it : it;
                 const int w = (q == h0 && h1 > 0) ? 1 : ((q == h0 + h1 && h2 > 0) ? 2 : -1);
                 segs[n++] = make_int4(it * stride, qe - q, w, q < n_guard ? it + 1 : 0);
                 q = qe;
             }
-            segs[7].x = n;
+            segs[11].x = n;
         }
     }
 
     const int n_stage = MODE >= KM_EULER ? (int)(A.n_steps * (MODE == KM_HEUN ? 2 : 1)) : 1;
+    // low-latency mode (resident step modes with several CTAs per system): the first granule of every stage comes
+    // from the tagged copy of the stream, word by word as the producers' stores land; the inter-CTA barrier is only
+    // passed later in the stage, before the rest of the stream is fetched by TMA
+    const bool use_ll = RESIDENT && stepping && A.n_cta > 1 && A.ll[0] != nullptr;
+    auto ll_of = [&](int k) { return reinterpret_cast<uint4 *>(A.ll[k & 1]) + (size_t)b * A.unit_stride * 6; };
     unsigned long long *bar = A.bar != nullptr ? A.bar + b : nullptr;
     unsigned long long bar_target = A.bar_base;
     bool probe_on = false;
@@ -418,7 +466,7 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
             dumbbell_force(x0, x1, stroke_length(tn, phs[sl], A.ell, A.lambda, A.omega), A.k0, F0);
 #pragma unroll
             for (int cc = 0; cc < 3; ++cc) { Fs[6 * sl + cc] = F0[cc]; Fs[6 * sl + 3 + cc] = -F0[cc]; }
-            publish_dumbbell(un, r0 + 2 * sl, x0, x1, F0);
+            publish_dumbbell(un, use_ll ? ll_of(A.cur) : nullptr, A.ll_tag0, r0 + 2 * sl, x0, x1, F0);
         }
         fence_proxy_async_global();   // the stream is also read through the async proxy (TMA)
     }
@@ -437,21 +485,26 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
         DS_PROBE(0);
         const T *units = reinterpret_cast<const T *>(A.units[(A.cur + g) & 1]) + (size_t)b * A.unit_stride * (6 * W);
 
-        if (tid == 0 && stepping && A.n_cta > 1) {
-            // inter-CTA barrier: every CTA of the system has published its rows of this stage's input
-            red_release_gpu(bar, 1ULL);
-            DS_PROBE(12);
-            bar_target += (unsigned long long)A.n_cta;
-            while (ld_relaxed_gpu(bar) < bar_target) {}
-            fence_acq_rel_gpu();
+        if (stepping && A.n_cta > 1) {
+            if (tid == 0) {
+                // inter-CTA barrier, arrival: this CTA has published its rows of this stage's input
+                red_release_gpu(bar, 1ULL);
+                DS_PROBE(12);
+                bar_target += (unsigned long long)A.n_cta;
+                if (!use_ll) {   // ... and wait: every CTA of the system has
+                    while (ld_relaxed_gpu(bar) < bar_target) {}
+                    fence_acq_rel_gpu();
+                }
+            }
         }
         DS_PROBE(1);
-        // stroke length at the end of this step, L(t_{n+1}), once per step (warps 1.. while warp 0 waits)
-        if (MODE >= KM_EULER && (MODE != KM_HEUN || (g & 1) == 0) && tid >= 32) {
+        // stroke length at the end of this step, L(t_{n+1}), once per step (lanes 1.. of warp 0, while thread 0 is busy
+        // with the barrier)
+        if (MODE >= KM_EULER && (MODE != KM_HEUN || (g & 1) == 0) && tid >= 1 && tid < 32) {
             const double t1 = time_of_step(A.t0, A.n0 + (MODE == KM_HEUN ? (g >> 1) : g) + 1, A.dt);
-            for (int sl = tid - 32; sl < nd; sl += NT - 32) Ls[sl] = stroke_length(t1, phs[sl], A.ell, A.lambda, A.omega);
+            for (int sl = tid - 1; sl < nd; sl += 31) Ls[sl] = stroke_length(t1, phs[sl], A.ell, A.lambda, A.omega);
         }
-        if (stepping && A.n_cta > 1) __syncthreads();   // the barrier has been passed (thread 0)
+        if (stepping && A.n_cta > 1 && !use_ll) __syncthreads();   // the barrier has been passed (thread 0)
         DS_PROBE(9);
 
         // alpha-spheres of this thread: rows 4 (q0 + ith) + k, rounded exactly as the stream rounds them
@@ -490,6 +543,19 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
                 cp_async16(sdst + a, gsrc + a);
             };
             const uint32_t par = (uint32_t)g & 1u;  // every granule barrier completes one phase per stage
+            // G1, G2: TMA bulk copies of consumption pieces [j0, j1) (two copies where the range wraps), thread 0
+            auto tma_range = [&](int j0, int j1, uint64_t *bar_) {
+                int a0 = sp + j0;
+                a0 = a0 >= tp ? a0 - tp : a0;
+                const int len = j1 - j0, first = a0 + len <= tp ? len : tp - a0;
+                mbar_expect_tx(bar_, (uint32_t)len * 16u);
+                bulk_g2s(sdst + a0, gsrc + a0, (uint32_t)first * 16u, bar_);
+                if (first < len) bulk_g2s(sdst, gsrc, (uint32_t)(len - first) * 16u, bar_);
+            };
+            auto issue_rest = [&]() {
+                if (h1 > 0) tma_range(pA, pAB, gran + 1);
+                if (h2 > 0) tma_range(pAB, tp, gran + 2);
+            };
             if (MODE == KM_APPLY && A.raw_pos != nullptr) {
                 // stateless apply: the CTA packs the user's arrays into its resident stream itself (no pack kernel,
                 // no global intermediate); CTAs start at different units so that they do not read L2 in a convoy
@@ -505,31 +571,50 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
                 mbar_arrive(gran + 0);
                 if (tid == 0) { mbar_arrive(gran + 1); mbar_arrive(gran + 2); }
             } else {
-                if (tid == 0) {   // G1, G2: TMA bulk copies of consumption pieces [j0, j1) (two copies where the range wraps)
-                    auto tma_range = [&](int j0, int j1, uint64_t *bar) {
-                        int a0 = sp + j0;
-                        a0 = a0 >= tp ? a0 - tp : a0;
-                        const int len = j1 - j0, first = a0 + len <= tp ? len : tp - a0;
-                        mbar_expect_tx(bar, (uint32_t)len * 16u);
-                        bulk_g2s(sdst + a0, gsrc + a0, (uint32_t)first * 16u, bar);
-                        if (first < len) bulk_g2s(sdst, gsrc, (uint32_t)(len - first) * 16u, bar);
-                    };
-                    if (h1 > 0) tma_range(pA, pAB, gran + 1);
-                    if (h2 > 0) tma_range(pAB, tp, gran + 2);
+                if (!use_ll) {
+                    if (tid == 0) issue_rest();
+                    for (int j = tid; j < pA; j += NT) copy_piece(j);   // G0: LDGSTS by every thread (lowest latency)
+                    cp_async_arrive(gran + 0);
+                } else {
+                    // G0 from the tagged copy: warps 1.. poll their pieces until the stage's tag shows in all four words
+                    if (tid >= 32) {
+                        const uint4 *lsrc = ll_of(A.cur + g);
+                        const uint32_t tag = A.ll_tag0 + (uint32_t)g;
+                        for (int j = tid - 32; j < pA; j += NT - 32) {
+                            int a = sp + j;
+                            a = a >= tp ? a - tp : a;
+                            uint4 w;
+                            if (a < 3 * A.U) {
+                                uint4 v0 = ld_volatile_v4(lsrc + 2 * a), v1 = ld_volatile_v4(lsrc + 2 * a + 1);
+                                while (v0.y != tag || v0.w != tag || v1.y != tag || v1.w != tag) {
+                                    const long long t_retry = clock64() + 256;   // back off: the pollers of 148 CTAs share the L2
+                                    while (clock64() < t_retry) {}
+                                    v0 = ld_volatile_v4(lsrc + 2 * a);
+                                    v1 = ld_volatile_v4(lsrc + 2 * a + 1);
+                                }
+                                w = make_uint4(v0.x, v0.z, v1.x, v1.z);
+                            } else {
+                                w = pad_piece<T>(a % 3);   // far-away zero-force unit of the stream's tail
+                            }
+                            sdst[a] = w;
+                        }
+                    }
+                    mbar_arrive(gran + 0);
                 }
-                for (int j = tid; j < pA; j += NT) copy_piece(j);   // G0: LDGSTS by every thread (lowest latency)
-                cp_async_arrive(gran + 0);
             }
             DS_PROBE(10);
             const V2<T> *const base = reinterpret_cast<const V2<T> *>(smem_raw) + 3 * jg;
             mbar_wait(gran + 0, par);
             DS_PROBE(2);
-            const int nseg = segs[7].x;
+            const int nseg = segs[11].x;
+            bool rest_issued = false;
+            unsigned long long bar_seen = 0;
             // the stage's total_it iterations (each: QI alpha x 1 unit per thread) as the few tight loops of the
             // segment table (built once, stage-invariant): {first piece, iterations, granule to wait for or -1,
             // first iteration + 1 if the segment holds own rows else 0}
             for (int sgi = 0; sgi < nseg; ++sgi) {
                 const int4 sg = segs[sgi];
+                if (use_ll && tid == 0 && !rest_issued) bar_seen = ld_relaxed_gpu(bar);   // consumed after the segment
                 if (sg.z >= 0) mbar_wait(gran + sg.z, par);
                 const V2<T> *p = base + sg.x;
                 if (sg.w != 0) {
@@ -547,6 +632,18 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
                 } else if (active) {
 #pragma unroll 1
                     for (int r = 0; r < sg.y; ++r, p += stride) pair_unit<T, TENSOR, false>(p, xi, acc, c1, negc2);
+                }
+                if (use_ll && tid == 0 && !rest_issued) {
+                    // low-latency mode: the inter-CTA barrier is passed here (every CTA has published this stage's
+                    // input, and nobody reads the buffers of two stages ago any more), then the rest of the stream is
+                    // fetched.  The counter was read when the segment began; only the last chance blocks.
+                    const bool last = sgi + 1 == nseg || segs[sgi + 1].z >= 0;
+                    if (bar_seen >= bar_target || last) {
+                        while (bar_seen < bar_target) bar_seen = ld_relaxed_gpu(bar);
+                        fence_acq_rel_gpu();
+                        issue_rest();
+                        rest_issued = true;
+                    }
                 }
             }
         } else {
@@ -672,7 +769,8 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
                     dumbbell_force(x0, x1, Ls[sl], A.k0, F0);
 #pragma unroll
                     for (int cc = 0; cc < 3; ++cc) { Fs[6 * sl + cc] = F0[cc]; Fs[6 * sl + 3 + cc] = -F0[cc]; }
-                    if (g + 1 < n_stage) publish_dumbbell(un, r0 + 2 * sl, x0, x1, F0);
+                    if (g + 1 < n_stage)
+                        publish_dumbbell(un, use_ll ? ll_of(A.cur + g + 1) : nullptr, A.ll_tag0 + (uint32_t)g + 1u, r0 + 2 * sl, x0, x1, F0);
                 }
                 fence_proxy_async_global();   // the stream is also read through the async proxy (TMA)
             }
