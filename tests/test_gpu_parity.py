@@ -272,3 +272,73 @@ def test_isolated_dumbbell_does_not_translate_on_gpu():
     w = inputs.Workload("single", X0, phi)
     Xg, _, _ = gpu_steps(w, ds.F64, 3000)
     assert np.abs(0.5 * (Xg[0, 0] + Xg[0, 1]) - np.array([3.0, -1.0, 2.0])).max() < 1e-12
+
+
+# --------------------------------------------------------------------------------- launch shapes of the step kernel
+@pytest.mark.parametrize("n_tiles", [1, 3, 17, 40, 96])
+def test_step_forced_tiles_cover_every_hand_over_mode(n_tiles):
+    """The persistent kernel under forced row tilings of one S = 192 system (N = 384): 1 CTA (no barrier),
+    3 CTAs (blocking barrier), 17+ CTAs (low-latency hand-over: tagged stream copy for the first granule, barrier
+    passed inside the stage), including shapes whose whole stream is the first granule."""
+    w = inputs.config5(B=1, S=192)
+    s, p = make_system(w, ds.F64)
+    with s:
+        s.set_tuning(n_tiles)
+        X0 = rounded(w, ds.F64)
+        s.set_state(dev(X0, ds.F64), torch.as_tensor(w.phase, device="cuda"), t0=0.1)
+        for c in (7, 1, 42):
+            s.step(c)
+        out = torch.empty((1, w.N, 3), dtype=torch.float64, device="cuda")
+        s.get_state(out)
+        V = torch.empty_like(out)
+        s.velocity(V)
+        torch.cuda.synchronize()
+    Xo = oracle.step(X0[0], w.phase[0], 0.1, 0, 50, p)
+    assert np.abs(out.cpu().numpy()[0] - Xo).max() <= 1e-10 * ELL
+    Vo = oracle.velocity(Xo, w.phase[0], 0.1 + 50 * p.dt, p)
+    assert rel_l2(V.cpu().numpy()[0], Vo) <= 1e-9
+
+
+def test_step_fp32_forced_tiles_low_latency():
+    w = inputs.config5(B=1, S=192)
+    Xg = {}
+    for n_tiles in (2, 48):
+        s, p = make_system(w, ds.F32)
+        with s:
+            s.set_tuning(n_tiles)
+            X0 = rounded(w, ds.F32)
+            s.set_state(dev(X0, ds.F32), torch.as_tensor(w.phase, device="cuda"))
+            s.step(300)
+            out = torch.empty((1, w.N, 3), dtype=torch.float32, device="cuda")
+            s.get_state(out)
+            torch.cuda.synchronize()
+            Xg[n_tiles] = out.cpu().numpy()[0].astype(np.float64)
+    Xo = oracle.step(X0[0], w.phase[0], 0.0, 0, 300, p)
+    for n_tiles in Xg:
+        assert np.abs(Xg[n_tiles] - Xo).max() <= 1e-4 * ELL
+
+
+def test_step_stream_larger_than_shared_memory():
+    """N = 16384 (FP32): the stage input (384 KB) does not fit a CTA's shared memory, so the step kernel streams it
+    through the TMA ring and keeps the blocking barrier; 2 Heun steps against the oracle."""
+    w = inputs.config5(B=1, S=8192)
+    Xg, X0, p = gpu_steps(w, ds.F32, 2)
+    Xo = oracle.step(X0[0], w.phase[0], 0.0, 0, 2, p)
+    assert np.abs(Xg[0] - Xo).max() <= 1e-4 * ELL
+
+
+def test_batch_more_systems_than_sms():
+    """B = 200 systems of S = 8: one CTA per system, any number of systems per launch."""
+    w = inputs.config5(B=200, S=8)
+    Xg, X0, p = gpu_steps(w, ds.F64, 100)
+    for b in (0, 77, 199):
+        Xo = oracle.step(X0[b], w.phase[b], 0.0, 0, 100, p)
+        assert np.abs(Xg[b] - Xo).max() <= 1e-10 * ELL
+
+
+def test_step_config4_fp32_1000_steps():
+    """north_star: FP32 trajectory within 1e-4 ell after 1000 steps, at the headline size (N = 4096)."""
+    w = inputs.config4()
+    Xg, X0, p = gpu_steps(w, ds.F32, 1000)
+    Xo = oracle.step(X0[0], w.phase[0], 0.0, 0, 1000, p)
+    assert np.abs(Xg[0] - Xo).max() <= 1e-4 * ELL
