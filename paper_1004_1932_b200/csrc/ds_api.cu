@@ -177,7 +177,7 @@ int choose_shape_step(ds_system *s) {
 bool stream_resident(int NQ, int U, int n_cta, int buf_bytes) {
     const int nq_lo = NQ / n_cta, nq_hi = (NQ + n_cta - 1) / n_cta;
     for (int nq = nq_lo < 1 ? 1 : nq_lo; nq <= nq_hi; ++nq) {
-        const int n_jg = ds::NT / nq;
+        const int n_jg = ds::NT / nq < U ? ds::NT / nq : U;
         const long long total_it = (U + n_jg - 1) / n_jg;
         if (total_it * n_jg * ds::UNIT_BYTES > buf_bytes) return false;
     }

@@ -346,7 +346,7 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
     // rows of this CTA and the (alpha-thread, beta-group) shape
     const int q0 = (int)((long long)c * A.NQ / A.n_cta), q1 = (int)((long long)(c + 1) * A.NQ / A.n_cta);
     const int nq = q1 - q0;                 // 1 .. NT (host guarantees)
-    const int n_jg = NT / nq;
+    const int n_jg = NT / nq < A.U ? NT / nq : A.U;   // beta-groups: no more than there are units
     const int ith = tid % nq, jg = tid / nq;
     const bool active = jg < n_jg;
     const int rows = 4 * nq;
@@ -441,6 +441,9 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
     // from the tagged copy of the stream, word by word as the producers' stores land; the inter-CTA barrier is only
     // passed later in the stage, before the rest of the stream is fetched by TMA
     const bool use_ll = RESIDENT && stepping && A.n_cta > 1 && A.ll[0] != nullptr;
+    // local mode (one CTA per system, resident): the stream never leaves shared memory; the stage's tail writes
+    // the next stage's units in place, no copy, no barrier
+    const bool local = RESIDENT && stepping && A.n_cta == 1;
     auto ll_of = [&](int k) { return reinterpret_cast<uint4 *>(A.ll[k & 1]) + (size_t)b * A.unit_stride * 6; };
     unsigned long long *bar = A.bar != nullptr ? A.bar + b : nullptr;
     unsigned long long bar_target = A.bar_base;
@@ -458,7 +461,9 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
             if (XcT != nullptr) XcT[e] = (T)Xs[e];
         }
         const double tn = time_of_step(A.t0, A.n0, A.dt);
-        T *un = reinterpret_cast<T *>(A.units[A.cur]) + (size_t)b * A.unit_stride * (6 * W);
+        T *un = local ? reinterpret_cast<T *>(smem_raw) : reinterpret_cast<T *>(A.units[A.cur]) + (size_t)b * A.unit_stride * (6 * W);
+        if (local)   // the tail of the stream: far-away zero-force pad units
+            for (int j = 3 * A.U + tid; j < tp; j += NT) reinterpret_cast<uint4 *>(smem_raw)[j] = pad_piece<T>(j % 3);
         for (int sl = tid; sl < nd; sl += NT) {
             double x0[3], x1[3], F0[3];
 #pragma unroll
@@ -556,7 +561,9 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
                 if (h1 > 0) tma_range(pA, pAB, gran + 1);
                 if (h2 > 0) tma_range(pAB, tp, gran + 2);
             };
-            if (MODE == KM_APPLY && A.raw_pos != nullptr) {
+            if (local) {
+                // the stream is in place (written by the previous stage's tail or the prologue)
+            } else if (MODE == KM_APPLY && A.raw_pos != nullptr) {
                 // stateless apply: the CTA packs the user's arrays into its resident stream itself (no pack kernel,
                 // no global intermediate); CTAs start at different units so that they do not read L2 in a convoy
                 typedef typename std::conditional<sizeof(T) == 4, float4, double2>::type Q;
@@ -604,7 +611,7 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
             }
             DS_PROBE(10);
             const V2<T> *const base = reinterpret_cast<const V2<T> *>(smem_raw) + 3 * jg;
-            mbar_wait(gran + 0, par);
+            if (!local) mbar_wait(gran + 0, par);
             DS_PROBE(2);
             const int nseg = segs[11].x;
             bool rest_issued = false;
@@ -615,7 +622,7 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
             for (int sgi = 0; sgi < nseg; ++sgi) {
                 const int4 sg = segs[sgi];
                 if (use_ll && tid == 0 && !rest_issued) bar_seen = ld_relaxed_gpu(bar);   // consumed after the segment
-                if (sg.z >= 0) mbar_wait(gran + sg.z, par);
+                if (sg.z >= 0 && !local) mbar_wait(gran + sg.z, par);
                 const V2<T> *p = base + sg.x;
                 if (sg.w != 0) {
                     // iterations that hold the CTA's own rows: a warp takes the guarded variant (r = 0 excluded)
@@ -761,7 +768,8 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
             DS_PROBE(17);
             // Eq. (4) at the new positions and time, one thread per dumbbell; publish the next stage's rows
             if (tid < ((nd + 31) & ~31)) {
-                T *un = reinterpret_cast<T *>(A.units[(A.cur + g + 1) & 1]) + (size_t)b * A.unit_stride * (6 * W);
+                T *un = local ? reinterpret_cast<T *>(smem_raw)
+                              : reinterpret_cast<T *>(A.units[(A.cur + g + 1) & 1]) + (size_t)b * A.unit_stride * (6 * W);
                 for (int sl = tid; sl < nd; sl += NT) {
                     double x0[3], x1[3], F0[3];
 #pragma unroll
@@ -774,6 +782,8 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
                 }
                 fence_proxy_async_global();   // the stream is also read through the async proxy (TMA)
             }
+            if (local)   // the pad units share their shared memory with the reduction scratch: rewrite them
+                for (int j = 3 * A.U + tid; j < tp; j += NT) reinterpret_cast<uint4 *>(smem_raw)[j] = pad_piece<T>(j % 3);
         }
         DS_PROBE(6);
         fence_proxy_async_shared();
