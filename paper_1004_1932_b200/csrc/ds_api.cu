@@ -150,7 +150,7 @@ int choose_shape_step(ds_system *s) {
             int per = s->num_sms / n;
             per = per < 1 ? 1 : (per > s->B ? s->B : per);
             const long long groups = (s->B + per - 1) / per;
-            const double cost = (double)groups * ((double)iters + (n > 1 ? 5.0 : 3.0));
+            const double cost = (double)groups * ((double)iters + (n > 1 ? 6.0 : 4.0));   // a stage's fixed part, in iterations: barrier + hand-over / local
             if (cost < best_cost * (1.0 - 1e-9)) { best_cost = cost; best = n; }
         }
     }

@@ -429,7 +429,8 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
                 int it = it_own + q;
                 it = it >= total_it ? it - total_it : it;
                 const int w = (q == h0 && h1 > 0) ? 1 : ((q == h0 + h1 && h2 > 0) ? 2 : -1);
-                segs[n++] = make_int4(it * stride, qe - q, w, q < n_guard ? it + 1 : 0);
+                const int tail = (it + (qe - q) == total_it) ? (1 << 30) : 0;   // the segment ends with the stream's last iteration
+                segs[n++] = make_int4(it * stride, (qe - q) | tail, w, q < n_guard ? it + 1 : 0);
                 q = qe;
             }
             segs[11].x = n;
@@ -610,7 +611,12 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
                 }
             }
             DS_PROBE(10);
-            const V2<T> *const base = reinterpret_cast<const V2<T> *>(smem_raw) + 3 * jg;
+            // groups take the units of an iteration in REVERSE order (group jg reads unit n_jg - 1 - jg), so that the
+            // pad units of the stream's last iteration fall to the low warps, which skip them: warp 0 also carries the
+            // barrier and the TMA issue
+            const int jgr = n_jg - 1 - jg;
+            const V2<T> *const base = reinterpret_cast<const V2<T> *>(smem_raw) + 3 * jgr;
+            const bool skip_tail = jgr >= A.U - (total_it - 1) * n_jg;   // this thread's unit of the last iteration is a pad
             if (!local) mbar_wait(gran + 0, par);
             DS_PROBE(2);
             const int nseg = segs[11].x;
@@ -624,21 +630,23 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
                 if (use_ll && tid == 0 && !rest_issued) bar_seen = ld_relaxed_gpu(bar);   // consumed after the segment
                 if (sg.z >= 0 && !local) mbar_wait(gran + sg.z, par);
                 const V2<T> *p = base + sg.x;
+                const int its = sg.y & 0xffffff;
+                const int its_mine = its - ((sg.y >> 30) && skip_tail ? 1 : 0);
                 if (sg.w != 0) {
                     // iterations that hold the CTA's own rows: a warp takes the guarded variant (r = 0 excluded)
                     // only if one of its lanes reads an own unit in that iteration
-                    int u = (sg.w - 1) * n_jg + jg;
+                    int u = (sg.w - 1) * n_jg + jgr;
 #pragma unroll 1
-                    for (int r = 0; r < sg.y; ++r, p += stride, u += n_jg) {
+                    for (int r = 0; r < its; ++r, p += stride, u += n_jg) {
                         const bool own = __any_sync(0xffffffffu, active && u >= d0 && u < d1);
-                        if (active) {
+                        if (active && r < its_mine) {
                             if (own) pair_unit<T, TENSOR, true>(p, xi, acc, c1, negc2);
                             else pair_unit<T, TENSOR, false>(p, xi, acc, c1, negc2);
                         }
                     }
                 } else if (active) {
 #pragma unroll 1
-                    for (int r = 0; r < sg.y; ++r, p += stride) pair_unit<T, TENSOR, false>(p, xi, acc, c1, negc2);
+                    for (int r = 0; r < its_mine; ++r, p += stride) pair_unit<T, TENSOR, false>(p, xi, acc, c1, negc2);
                 }
                 if (use_ll && tid == 0 && !rest_issued) {
                     // low-latency mode: the inter-CTA barrier is passed here (every CTA has published this stage's
@@ -711,10 +719,23 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
                 if (task < n_task) {
                     const int tq = task / 3, mq = task - 3 * tq;        // quad, which 4 of its 12 elements
                     const typename P::T4 *rp = reinterpret_cast<const typename P::T4 *>(red + 12 * tq + 4 * mq);
-                    for (int gq = my_part; gq < n_jg; gq += RP) {
-                        const typename P::T4 v = rp[3 * nq * gq];
-                        s0 += v.x; s1 += v.y; s2 += v.z; s3 += v.w;
+                    // two independent partial sums per element, loads four groups ahead of the adds
+                    T t0 = T(0), t1 = T(0), t2 = T(0), t3 = T(0);
+                    const int gstep = 3 * nq * RP;
+                    rp += 3 * nq * my_part;
+                    int gq = my_part;
+                    for (; gq + 3 * RP < n_jg; gq += 4 * RP, rp += 4 * gstep) {
+                        const typename P::T4 a = rp[0], bq = rp[gstep], cq = rp[2 * gstep], dq = rp[3 * gstep];
+                        s0 += a.x; s1 += a.y; s2 += a.z; s3 += a.w;
+                        t0 += bq.x; t1 += bq.y; t2 += bq.z; t3 += bq.w;
+                        s0 += cq.x; s1 += cq.y; s2 += cq.z; s3 += cq.w;
+                        t0 += dq.x; t1 += dq.y; t2 += dq.z; t3 += dq.w;
                     }
+                    for (; gq < n_jg; gq += RP, rp += gstep) {
+                        const typename P::T4 a = rp[0];
+                        s0 += a.x; s1 += a.y; s2 += a.z; s3 += a.w;
+                    }
+                    s0 += t0; s1 += t1; s2 += t2; s3 += t3;
                 }
                 DS_PROBE(18);
 #pragma unroll
