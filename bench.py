@@ -129,6 +129,7 @@ def time_steps(torch, ds, w, precision, tensor, n_steps, warmup, ranks=None, sam
         step(int(n_steps))
         e1.record(stream)
         torch.cuda.synchronize()
+        launches = s.launch_count() - l0      # kernels launched inside the timed region
         if sampler is not None:
             sampler.__exit__()
         if ranks is not None:
@@ -138,7 +139,7 @@ def time_steps(torch, ds, w, precision, tensor, n_steps, warmup, ranks=None, sam
         torch.cuda.synchronize()
         if not bool(torch.isfinite(out).all()):
             raise RuntimeError("non-finite state after the timed steps")
-        return e0.elapsed_time(e1) * 1e-3, s.launch_count() - l0
+        return e0.elapsed_time(e1) * 1e-3, launches
 
 
 def time_steps_cold_l2(torch, ds, w, precision, tensor, n_steps):
