@@ -405,9 +405,10 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
     // 48-byte thread stride: conflict-free); the sums of quad ith are elements 12 ith + m of the CTA's state.
     // A task = (quad ith, 4 consecutive m) is summed by RP consecutive lanes: lane part adds the groups
     // jg = part, part + RP, ... with one LDS.128 each, then log2(RP) shuffle steps.
-    constexpr int RP = 8;
+    const int rp_log = n_jg >= 32 ? 3 : (n_jg >= 16 ? 2 : (n_jg >= 8 ? 1 : 0));   // few groups: fewer lanes per task, more tasks per pass
+    const int RP = 1 << rp_log, tpw = 32 >> rp_log;                              // lanes per task, tasks per warp
     const int n_task = 3 * nq;                                  // tasks of the CTA
-    const int my_task = tid / RP, my_part = tid % RP;
+    const int my_task = tid >> rp_log, my_part = tid & (RP - 1);
     if (tid == 0) {
         for (int s = 0; s < NS_MAX; ++s) {
             mbar_init(full + s, 1);
@@ -714,7 +715,7 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
         DS_PROBE(5);
         if (tid < ((n_task * RP + 31) & ~31)) {        // the warps that hold tasks
             const bool pred = MODE == KM_HEUN && (g & 1) == 0, corr = MODE == KM_HEUN && (g & 1) == 1;
-            for (int task = my_task; task < ((n_task + 3) & ~3); task += NT / RP) {   // warp-uniform trip count (4 tasks per warp)
+            for (int task = my_task; task < ((n_task + tpw - 1) & ~(tpw - 1)); task += NT >> rp_log) {   // warp-uniform trip count
                 T s0 = T(0), s1 = T(0), s2 = T(0), s3 = T(0);
                 if (task < n_task) {
                     const int tq = task / 3, mq = task - 3 * tq;        // quad, which 4 of its 12 elements
@@ -739,9 +740,11 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
                 }
                 DS_PROBE(18);
 #pragma unroll
-                for (int d = 1; d < RP; d <<= 1) {
-                    s0 += __shfl_xor_sync(0xffffffffu, s0, d); s1 += __shfl_xor_sync(0xffffffffu, s1, d);
-                    s2 += __shfl_xor_sync(0xffffffffu, s2, d); s3 += __shfl_xor_sync(0xffffffffu, s3, d);
+                for (int d = 1; d < 8; d <<= 1) {
+                    if (d < RP) {   // CTA-uniform
+                        s0 += __shfl_xor_sync(0xffffffffu, s0, d); s1 += __shfl_xor_sync(0xffffffffu, s1, d);
+                        s2 += __shfl_xor_sync(0xffffffffu, s2, d); s3 += __shfl_xor_sync(0xffffffffu, s3, d);
+                    }
                 }
                 DS_PROBE(19);
                 if (my_part != 0 || task >= n_task) continue;
