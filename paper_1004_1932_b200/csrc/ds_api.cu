@@ -252,9 +252,9 @@ int launch_state_run(ds_system *s, int mode, long long n_steps, void *out_u) {
     A.n0 = s->n_host; A.n_steps = n_steps; A.out_u = out_u;
     A.X = s->X; A.phase = s->phase;
     A.bar = s->bar; A.bar_base = s->bar_base;
-    // low-latency stage hand-over (tagged stream copy) pays off when many CTAs meet at the barrier (measured: 147 CTAs
-    // -9 % per stage, 2 CTAs +5 %)
-    const bool low_latency = s->n_cta > 16;
+    // low-latency stage hand-over (tagged stream copy) whenever CTAs meet at a barrier (measured per stage: 147 CTAs -9 %,
+    // 16 CTAs -10 %, 4 CTAs -15 %, 2 CTAs -1 %)
+    const bool low_latency = s->n_cta > 1;
     A.ll[0] = low_latency ? s->ll[0] : nullptr; A.ll[1] = low_latency ? s->ll[1] : nullptr;
     A.h0_ll = 4;
     A.state_smem = s->state_smem; A.Xcg = s->Xcg; A.V1g = s->V1g; A.Fg = s->Fg; A.Lg = s->Lg;
