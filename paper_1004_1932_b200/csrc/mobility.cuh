@@ -414,7 +414,8 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
             mbar_init(full + s, 1);
             mbar_init(empty + s, NT / 32);
         }
-        mbar_init(gran + 0, NT);   // G0: every thread's LDGSTS copies
+        // G0: every thread's LDGSTS copies; in low-latency mode warps 1.. fill G0 and warp 0 (barrier arrival) only waits
+        mbar_init(gran + 0, (RESIDENT && MODE != KM_APPLY && A.n_cta > 1 && A.ll[0] != nullptr) ? NT - 32 : NT);
         mbar_init(gran + 1, 1);    // G1, G2: thread 0's TMA bulk copies
         mbar_init(gran + 2, 1);
         mbar_fence_init();
@@ -607,8 +608,8 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
                             }
                             sdst[a] = w;
                         }
+                        mbar_arrive(gran + 0);
                     }
-                    mbar_arrive(gran + 0);
                 }
             }
             DS_PROBE(10);
