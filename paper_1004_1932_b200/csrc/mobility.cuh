@@ -2,35 +2,38 @@
 // part with the tensor of Eq. (3a,3b), fused with the O(N) rest of the time
 // step (self term, reduction, integrator update, next force evaluation) and
 // with the step loop itself: ONE launch runs all n_steps of ds_step / ds_batch_step.
+// (DESIGN.md section 6 is the long form of this comment.)
 //
 // Decomposition ("row owner": no partial sum ever leaves the SM).
 //   grid = (n_cta row tiles, systems), one CTA of NT = 512 threads per SM.
 //   The N alpha-spheres of a system are cut into NQ = ceil(N/4) quads; CTA c owns the contiguous
-//   quads [c NQ / n_cta, (c+1) NQ / n_cta) -- nq of them, chosen by the host so that
-//   systems * n_cta fills the 148 SMs (N = 4096: 148 CTAs of 6 or 7 quads).
-//   Thread t = (ith, jg) = (t % nq, t / nq): it keeps the I = 4 alpha-spheres of quad q0 + ith in
-//   registers and belongs to beta-group jg of n_jg = NT / nq.  The split over beta is therefore
-//   INSIDE the CTA; it is undone through shared memory in a fixed order (deterministic, no
-//   floating-point atomics, no global scratch).
-//   Every CTA streams ALL beta-spheres of its system through a ring of shared-memory slots filled
-//   by TMA bulk copies (cp.async.bulk global -> shared, completion on an mbarrier; one elected
-//   thread issues them, consumer warps release slots through a second mbarrier).  The beta-stream
-//   lives in global memory (L2-resident) in the exact shared-memory layout ("units", see pack.cuh):
-//   one unit = W beta-spheres = 6 packs = 48 bytes, so a chunk is one contiguous copy.  N = 4096
-//   (FP32: 96 KB, FP64: 192 KB) is resident at once: all copies are issued up front.
-//   Inside a chunk, group jg takes units jg, jg + n_jg, ... (consecutive groups read consecutive
-//   48-byte units: conflict-free LDS.128, broadcast within a group); a chunk holds a multiple of
-//   n_jg units (the stream is padded with far-away zero-force units), so every thread of the CTA
-//   makes the same number of iterations.
-//   r = 0 (alpha == beta) is excluded by a guarded rsqrt compiled only into the loop variant used
-//   for chunks that intersect the CTA's own rows (CTA-uniform choice).
+//   quads [c NQ / n_cta, (c+1) NQ / n_cta) -- nq of them (N = 4096: 147 CTAs of 7 or 6 quads).
+//   Thread t = (ith, jg) = (t % nq, t / nq): it keeps the 4 alpha-spheres of quad q0 + ith in
+//   registers and belongs to beta-group jg of n_jg = min(NT / nq, units).  The split over beta is
+//   therefore INSIDE the CTA; it is undone through shared memory and shuffles in a fixed order
+//   (deterministic, no floating-point atomics, no global scratch).
+//   Every CTA walks ALL beta-spheres of its system.  The beta-stream lives in global memory
+//   (L2-resident) in the exact shared-memory layout ("units", see pack.cuh): one unit = W
+//   beta-spheres = 6 packs = 48 bytes; it ends with far-away zero-force pad units.  One iteration =
+//   4 alpha x 1 unit per thread; the groups of an iteration read consecutive 48-byte units
+//   (conflict-free LDS.128, broadcast within a group).
+//     RESIDENT (the stream fits the CTA's shared memory: N <= 8192 FP32 / 4096 FP64): the stream sits in
+//       shared memory in natural order and is consumed starting at the CTA's own rows, in three granules:
+//       G0 by every thread (LDGSTS, or the tagged low-latency copy, see below), G1 and G2 by TMA bulk copies.
+//     otherwise: a ring of 24 KB slots filled by TMA bulk copies (cp.async.bulk, completion on an mbarrier;
+//       one thread issues them, consumer warps release slots through a second mbarrier).
+//   r = 0 (alpha == beta) is excluded by a guarded rsqrt compiled only into the loop variant taken by the
+//   warps that read an own unit, in the one or two iterations that hold the CTA's own rows.
 //
-// Time stepping (RUN_STEP).  The CTA keeps its rows' state (X_n, V1, F; FP64) in shared memory for
-// the whole launch.  A stage = pair sum over the input stream -> reduction -> Eq. (3a) self term ->
-// integrator update -> Eq. (4) at the new positions -> publish the CTA's rows of the next stage's
-// stream (ping-pong buffer in global memory) -> inter-CTA barrier (one arrival counter per system,
-// release/acquire at gpu scope; the grid is launched cooperatively so all CTAs are co-resident).
+// Time stepping.  The CTA keeps its rows' state (X_n, the stage's positions, V1, F; FP64) in shared
+// memory for the whole launch.  A stage = pair sum over the input stream -> reduction -> Eq. (3a) self
+// term -> integrator update -> Eq. (4) at the new positions -> publish the CTA's rows of the next
+// stage's stream (ping-pong buffers in global memory, plain and tagged copy) -> inter-CTA barrier (one
+// arrival counter per system, release/acquire at gpu scope; the grid is launched cooperatively so all
+// CTAs are co-resident).  In low-latency mode the first granule of the next stage is read from the
+// tagged copy as soon as the producers' stores land, and the barrier is passed later inside the stage.
 // Heun = 2 stages per step, Euler = 1.  No host round trip, no kernel boundary per step.
+// One CTA per system (local mode): the stream never leaves shared memory.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -66,7 +69,7 @@ struct RunArgs {
     int b0;                   // first system of this launch (blockIdx.y is relative to it)
     long long unit_stride;    // units per system in the streams (>= U + PAD_UNITS)
     void *units[2];           // beta-streams T[B][unit_stride][6][W]; stage g reads units[(cur+g)&1]
-    int cur;
+    int cur;                  // always 0 today (the prologue republishes the stream of the first stage)
     // Eq. (3) constants
     double self_mob;  // 1/(6 pi eta a)   Eq. (3a)
     double pre;       // 1/(8 pi eta)     Eq. (3b)
