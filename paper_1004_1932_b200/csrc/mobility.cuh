@@ -146,6 +146,11 @@ __device__ __forceinline__ unsigned long long ld_relaxed_gpu(const unsigned long
     return v;
 }
 __device__ __forceinline__ void fence_acq_rel_gpu() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
+__device__ __forceinline__ unsigned long long ld_acquire_gpu(const unsigned long long *p) {
+    unsigned long long v;
+    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
 // Ampere-style asynchronous copy, 16 bytes global (L2 only, .cg) -> shared, in the generic proxy (SASS: LDGSTS);
 // the mbarrier form makes `bar` count this thread's arrival once all its earlier copies have landed
 __device__ __forceinline__ void cp_async16(void *dst, const void *src) {
@@ -497,11 +502,11 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
         const T *units = reinterpret_cast<const T *>(A.units[(A.cur + g) & 1]) + (size_t)b * A.unit_stride * (6 * W);
 
         if (stepping && A.n_cta > 1) {
+            bar_target += (unsigned long long)A.n_cta;
             if (tid == 0) {
                 // inter-CTA barrier, arrival: this CTA has published its rows of this stage's input
                 red_release_gpu(bar, 1ULL);
                 DS_PROBE(12);
-                bar_target += (unsigned long long)A.n_cta;
                 if (!use_ll) {   // ... and wait: every CTA of the system has
                     while (ld_relaxed_gpu(bar) < bar_target) {}
                     fence_acq_rel_gpu();
@@ -632,7 +637,7 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
             // first iteration + 1 if the segment holds own rows else 0}
             for (int sgi = 0; sgi < nseg; ++sgi) {
                 const int4 sg = segs[sgi];
-                if (use_ll && tid == 0 && !rest_issued) bar_seen = ld_relaxed_gpu(bar);   // consumed after the segment
+                if (use_ll && tid == 32 && !rest_issued) bar_seen = ld_acquire_gpu(bar);   // consumed after the segment
                 if (sg.z >= 0 && !local) mbar_wait(gran + sg.z, par);
                 const V2<T> *p = base + sg.x;
                 const int its = sg.y & 0xffffff;
@@ -653,14 +658,13 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
 #pragma unroll 1
                     for (int r = 0; r < its_mine; ++r, p += stride) pair_unit<T, TENSOR, false>(p, xi, acc, c1, negc2);
                 }
-                if (use_ll && tid == 0 && !rest_issued) {
+                if (use_ll && tid == 32 && !rest_issued) {   // warp 1: warp 0 already carries the arrival
                     // low-latency mode: the inter-CTA barrier is passed here (every CTA has published this stage's
                     // input, and nobody reads the buffers of two stages ago any more), then the rest of the stream is
                     // fetched.  The counter was read when the segment began; only the last chance blocks.
                     const bool last = sgi + 1 == nseg || segs[sgi + 1].z >= 0;
                     if (bar_seen >= bar_target || last) {
-                        while (bar_seen < bar_target) bar_seen = ld_relaxed_gpu(bar);
-                        fence_acq_rel_gpu();
+                        while (bar_seen < bar_target) bar_seen = ld_acquire_gpu(bar);   // acquire: pairs with every CTA's red.release
                         issue_rest();
                         rest_issued = true;
                     }
