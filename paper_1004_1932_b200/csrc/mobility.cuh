@@ -427,6 +427,8 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
         mbar_init(gran + 1, 1);    // G1, G2: thread 0's TMA bulk copies
         mbar_init(gran + 2, 1);
         mbar_fence_init();
+    }
+    if (tid == 64) {   // another warp than the one that initialises the barriers
         if (RESIDENT) {
             // a new tight loop starts where a granule begins, where the guard ends and where the stream wraps around
             const int wrapq = total_it - it_own;
@@ -486,7 +488,8 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
         }
         fence_proxy_async_global();   // the stream is also read through the async proxy (TMA)
     }
-    __syncthreads();  // mbarriers initialised; state and published rows written
+    if (!(MODE == KM_APPLY && RESIDENT && A.raw_pos != nullptr))
+        __syncthreads();  // mbarriers initialised; state and published rows written (the in-kernel pack of the apply ends with its own)
 
 
     // ring mode: k-th chunk in this CTA's consumption order -> chunk index, iterations; ring position of the next
