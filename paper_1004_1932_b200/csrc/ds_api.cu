@@ -195,6 +195,17 @@ int launch_run_v(ds_system *s, ds::RunArgs &A, dim3 grid, size_t smem, bool coop
     if (coop) {
         void *args[] = {(void *)&A};
         CU_TRY(cudaLaunchCooperativeKernel((const void *)kern, grid, dim3(ds::NT), args, smem, st));
+    } else if (MODE == ds::KM_APPLY) {
+        // programmatic dependent launch: the CTAs of this apply may become resident while the previous kernel of the
+        // stream drains; the kernel waits (griddepcontrol.wait) before its first global access
+        cudaLaunchConfig_t cfg;
+        memset(&cfg, 0, sizeof cfg);
+        cfg.gridDim = grid; cfg.blockDim = dim3(ds::NT); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        CU_TRY(cudaLaunchKernelEx(&cfg, kern, A));
     } else {
         kern<<<grid, dim3(ds::NT), smem, st>>>(A);
         CU_TRY(cudaGetLastError());

@@ -449,6 +449,12 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
         }
     }
 
+    if (MODE == KM_APPLY) {
+        // programmatic dependent launch (ds_api.cu): let the next kernel of the stream become resident as SMs free up,
+        // and do not touch global memory before the previous kernel has completed
+        asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+        asm volatile("griddepcontrol.wait;" ::: "memory");
+    }
     const int n_stage = MODE >= KM_EULER ? (int)(A.n_steps * (MODE == KM_HEUN ? 2 : 1)) : 1;
     // low-latency mode (resident step modes with several CTAs per system): the first granule of every stage comes
     // from the tagged copy of the stream, word by word as the producers' stores land; the inter-CTA barrier is only
