@@ -342,3 +342,14 @@ def test_step_config4_fp32_1000_steps():
     Xg, X0, p = gpu_steps(w, ds.F32, 1000)
     Xo = oracle.step(X0[0], w.phase[0], 0.0, 0, 1000, p)
     assert np.abs(Xg[0] - Xo).max() <= 1e-4 * ELL
+
+
+def test_apply_scaling_sweep_65536_full_size():
+    """BASELINE.json config 5, the largest sweep member N = 65536 (FP32, RPY), in the launch configuration bench.py
+    times (pack kernel + TMA ring, several waves): every output against the oracle (4.3e9 pair evaluations)."""
+    X, F = inputs.sweep_case(16)
+    u = gpu_apply(X, F, ds.F32, ds.RPY)
+    ref = oracle_apply(X, F, ds.F32, ds.RPY)
+    assert rel_l2(u, ref) <= TOL[ds.F32]
+    scale = np.sqrt(np.mean(ref ** 2))
+    assert np.abs(u - ref).max() <= 20 * TOL[ds.F32] * scale
