@@ -67,6 +67,8 @@ struct ds_system {
     int64_t launches = 0;
     // state
     double *X = nullptr, *phase = nullptr;
+    void *xu = nullptr;                         // the positions in user precision [B][N][3] (host-buffer fast path)
+    bool x_valid = false, xu_valid = false;     // which of X (FP64) / xu holds the current state (at least one does)
     void *units[2] = {nullptr, nullptr};        // beta-streams (mobility.cuh), ping-pong over the stages
     unsigned long long *bar = nullptr;          // [B] arrival counters of the inter-CTA barrier
     unsigned long long bar_base = 0;
@@ -261,7 +263,7 @@ int launch_state_run(ds_system *s, int mode, long long n_steps, void *out_u) {
     fill_constants(s, A);
     A.mode = mode; A.heun = s->P.integrator == DS_HEUN ? 1 : 0;
     A.n0 = s->n_host; A.n_steps = n_steps; A.out_u = out_u;
-    A.X = s->X; A.phase = s->phase;
+    A.X = s->X; A.phase = s->phase; A.xu = s->xu; A.from_user = s->x_valid ? 0 : 1;
     A.bar = s->bar; A.bar_base = s->bar_base;
     // low-latency stage hand-over (tagged stream copy) whenever CTAs meet at a barrier (measured per stage: 147 CTAs -9 %,
     // 16 CTAs -10 %, 4 CTAs -15 %, 2 CTAs -1 %)
@@ -286,6 +288,7 @@ int launch_state_run(ds_system *s, int mode, long long n_steps, void *out_u) {
     }
     if (s->n_cta > 1) s->bar_base += (unsigned long long)s->n_cta * (unsigned long long)n_stage;
     s->ll_tag += (unsigned int)n_stage + 1u;
+    if (mode == ds::RUN_STEP) { s->x_valid = true; s->xu_valid = true; }   // the kernel leaves the state in both forms
     return DS_OK;
 }
 
@@ -354,6 +357,14 @@ template <typename T> int peak_probe_t(int num_sms, double *flops_per_s) {
 
 bool finite_pos(double x) { return isfinite(x) && x > 0.0; }
 
+// X (FP64) <- xu (user precision) when only the latter is current (ds_set_state with a host buffer)
+int materialize_x(ds_system *s) {
+    if (s->x_valid) return DS_OK;
+    DS_TRY(s->P.precision == DS_F64 ? run_state_init<double>(s, s->xu) : run_state_init<float>(s, s->xu));
+    s->x_valid = true;
+    return DS_OK;
+}
+
 }  // namespace
 
 // =================================================================================================
@@ -418,6 +429,7 @@ int ds_create(const ds_params *p, ds_system **out) {
     cudaError_t e = cudaSuccess;
     auto al = [&](void **ptr, size_t bytes) { if (e == cudaSuccess) e = cudaMalloc(ptr, bytes); };
     al((void **)&s->X, n3 * 8);
+    al(&s->xu, n3 * (f64 ? 8 : 4));
     al((void **)&s->phase, (size_t)s->B * s->S * 8);
     al(&s->units[0], ub); al(&s->units[1], ub);
     al(&s->ll[0], 2 * ub); al(&s->ll[1], 2 * ub);
@@ -440,7 +452,7 @@ int ds_destroy(ds_system *s) {
     if (!s) return DS_OK;
     cudaSetDevice(s->P.device);
     cudaStreamSynchronize(s->stream);
-    void *ptrs[] = {s->X, s->phase, s->units[0], s->units[1], s->ll[0], s->ll[1], s->bar, s->Xcg, s->V1g, s->Fg, s->Lg,
+    void *ptrs[] = {s->X, s->xu, s->phase, s->units[0], s->units[1], s->ll[0], s->ll[1], s->bar, s->Xcg, s->V1g, s->Fg, s->Lg,
                     s->ap_units.p, s->st_a.p, s->st_b.p, s->st_c.p};
     for (void *q : ptrs) if (q) cudaFree(q);
     (void)cudaGetLastError();
@@ -480,15 +492,16 @@ int ds_set_state(ds_system *s, const void *pos, const void *phase, double t0) {
     DS_TRY(is_device_ptr(phase, &dev));
     CU_TRY(cudaMemcpyAsync(s->phase, phase, pb, dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s->stream));
     DS_TRY(is_device_ptr(pos, &dev));
-    const void *dpos = pos;
-    if (!dev) {
-        DS_TRY(ensure(s->st_a, nb));
-        CU_TRY(cudaMemcpyAsync(s->st_a.p, pos, nb, cudaMemcpyHostToDevice, s->stream));
-        dpos = s->st_a.p;
-    }
     s->t0 = t0;
     s->n_host = 0;
-    DS_TRY(s->P.precision == DS_F64 ? run_state_init<double>(s, dpos) : run_state_init<float>(s, dpos));
+    if (!dev) {
+        // host buffer: one copy into the user-precision image; the next kernel widens it to FP64 itself
+        CU_TRY(cudaMemcpyAsync(s->xu, pos, nb, cudaMemcpyHostToDevice, s->stream));
+        s->xu_valid = true; s->x_valid = false;
+    } else {
+        DS_TRY(s->P.precision == DS_F64 ? run_state_init<double>(s, pos) : run_state_init<float>(s, pos));
+        s->x_valid = true; s->xu_valid = false;
+    }
     s->has_state = true;
     return DS_OK;
 }
@@ -502,19 +515,18 @@ int ds_get_state(ds_system *s, void *pos, double *t) {
     const size_t es = elem_size(s), nb = (size_t)s->B * s->N * 3 * es;
     int dev = 0;
     DS_TRY(is_device_ptr(pos, &dev));
-    void *dpos = pos;
-    if (!dev) { DS_TRY(ensure(s->st_c, nb)); dpos = s->st_c.p; }
-    const long long n3 = (long long)s->B * s->N * 3;
-    if (s->P.precision == DS_F64)
-        ds::state_out_kernel<double><<<(unsigned)((n3 + 255) / 256), 256, 0, s->stream>>>(s->X, dpos, n3);
-    else
-        ds::state_out_kernel<float><<<(unsigned)((n3 + 255) / 256), 256, 0, s->stream>>>(s->X, dpos, n3);
-    CU_TRY(cudaGetLastError());
-    s->launches += 1;
-    if (!dev) {
-        CU_TRY(cudaMemcpyAsync(pos, dpos, nb, cudaMemcpyDeviceToHost, s->stream));
-        CU_TRY(cudaStreamSynchronize(s->stream));
+    if (!s->xu_valid) {   // user-precision image of X
+        const long long n3 = (long long)s->B * s->N * 3;
+        if (s->P.precision == DS_F64)
+            ds::state_out_kernel<double><<<(unsigned)((n3 + 255) / 256), 256, 0, s->stream>>>(s->X, s->xu, n3);
+        else
+            ds::state_out_kernel<float><<<(unsigned)((n3 + 255) / 256), 256, 0, s->stream>>>(s->X, s->xu, n3);
+        CU_TRY(cudaGetLastError());
+        s->launches += 1;
+        s->xu_valid = true;
     }
+    CU_TRY(cudaMemcpyAsync(pos, s->xu, nb, dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, s->stream));
+    if (!dev) CU_TRY(cudaStreamSynchronize(s->stream));
     return DS_OK;
 }
 
@@ -527,6 +539,7 @@ int ds_forces(ds_system *s, void *F) {
     DS_TRY(is_device_ptr(F, &dev));
     void *dF = F;
     if (!dev) { DS_TRY(ensure(s->st_c, nb)); dF = s->st_c.p; }
+    DS_TRY(materialize_x(s));
     DS_TRY(s->P.precision == DS_F64 ? run_forces_out<double>(s, dF) : run_forces_out<float>(s, dF));
     if (!dev) {
         CU_TRY(cudaMemcpyAsync(F, dF, nb, cudaMemcpyDeviceToHost, s->stream));

@@ -82,6 +82,8 @@ struct RunArgs {
     void *out_u;              // RUN_APPLY / RUN_VELOCITY: u [B][N][3] user precision
     const void *raw_pos, *raw_F;  // RUN_APPLY with a resident stream: the user's [n][3] arrays (each CTA packs them itself)
     double *X;                // state positions [B][N][3] (read at start; written at the end of RUN_STEP)
+    void *xu;                 // the same in user precision [B][N][3]: written at the end of RUN_STEP (ds_get_state reads it);
+    int from_user;            // 1: the launch starts from xu (ds_set_state with a host buffer left X stale)
     const double *phase;      // [B][S]
     double t0, dt, ell, lambda, omega, k0;
     // inter-CTA barrier: one monotonic arrival counter per system; this launch starts at bar_base
@@ -470,8 +472,11 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
 
     // ---- prologue of the step modes: own rows X -> state, F(X_n, t_n), publish the stream rows ----
     if (stepping) {
+        if (!A.state_smem && A.from_user)
+            for (int e = tid; e < 3 * nrows; e += NT) Xs[e] = (double)reinterpret_cast<const T *>(A.xu)[sys3 + 3 * r0 + e];
         if (A.state_smem) {
-            for (int e = tid; e < 3 * nrows; e += NT) Xs[e] = A.X[sys3 + 3 * r0 + e];
+            for (int e = tid; e < 3 * nrows; e += NT)
+                Xs[e] = A.from_user ? (double)reinterpret_cast<const T *>(A.xu)[sys3 + 3 * r0 + e] : A.X[sys3 + 3 * r0 + e];
             for (int sl = tid; sl < nd; sl += NT) const_cast<double *>(phs)[sl] = A.phase[(size_t)b * (A.N / 2) + (r0 >> 1) + sl];
         }
         __syncthreads();
@@ -832,8 +837,13 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
         DS_PROBE(7);
     }
 
-    if (MODE >= KM_EULER && A.state_smem)
-        for (int e = tid; e < 3 * nrows; e += NT) A.X[sys3 + 3 * r0 + e] = Xs[e];
+    if (MODE >= KM_EULER) {   // the state leaves the launch in FP64 and in user precision
+        for (int e = tid; e < 3 * nrows; e += NT) {
+            const double x = Xs[e];
+            if (A.state_smem) A.X[sys3 + 3 * r0 + e] = x;
+            reinterpret_cast<T *>(A.xu)[sys3 + 3 * r0 + e] = (T)x;
+        }
+    }
 }
 
 }  // namespace ds

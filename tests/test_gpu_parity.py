@@ -353,3 +353,41 @@ def test_apply_scaling_sweep_65536_full_size():
     assert rel_l2(u, ref) <= TOL[ds.F32]
     scale = np.sqrt(np.mean(ref ** 2))
     assert np.abs(u - ref).max() <= 20 * TOL[ds.F32] * scale
+
+
+@pytest.mark.parametrize("precision", [ds.F32, ds.F64])
+def test_host_buffers_state_path_matches_device_buffers(precision):
+    """ds_set_state / ds_get_state / ds_forces / ds_velocity with HOST buffers (the library keeps a user-precision image
+    of the state; the next kernel widens it) give bit-identical results to the device-buffer path, in any call order."""
+    w = inputs.config2()
+    X0 = np.ascontiguousarray(rounded(w, precision), dtype=NPDT[precision])
+    ph = np.ascontiguousarray(w.phase)
+    res = {}
+    for host in (False, True):
+        s, p = make_system(w, precision)
+        with s:
+            def buf():
+                return np.empty((w.B, w.N, 3), dtype=NPDT[precision]) if host else \
+                    torch.empty((w.B, w.N, 3), dtype=TDT[precision], device="cuda")
+
+            def val(b):
+                torch.cuda.synchronize()
+                return np.array(b if host else b.cpu().numpy(), dtype=np.float64)
+            s.set_state(X0 if host else dev(X0, precision), ph if host else torch.as_tensor(ph, device="cuda"), t0=0.2)
+            g0 = buf(); s.get_state(g0)                       # before any kernel touched the state
+            v0 = buf(); s.velocity(v0)
+            f0 = buf(); s.forces(f0)
+            s.step(25)
+            f1 = buf(); s.forces(f1)
+            g1 = buf(); t = s.get_state(g1)
+            s.set_state(X0 if host else dev(X0, precision), ph if host else torch.as_tensor(ph, device="cuda"), t0=0.2)
+            s.step(25)                                        # straight from set_state into the step kernel
+            g2 = buf(); s.get_state(g2)
+            res[host] = [val(x) for x in (g0, v0, f0, f1, g1, g2)]
+            assert t == pytest.approx(0.2 + 25 * p.dt)
+    for a, b_ in zip(res[False], res[True]):
+        assert np.array_equal(a, b_)
+    assert np.array_equal(res[True][0], X0.astype(np.float64))
+    assert np.array_equal(res[True][4], res[True][5])
+    Xo = oracle.step(X0[0].astype(np.float64), ph[0], 0.2, 0, 25, p)
+    assert np.abs(res[True][4][0] - Xo).max() <= (1e-4 if precision == ds.F32 else 1e-10) * ELL
