@@ -63,6 +63,9 @@ def lib():
         L.or_step_record.argtypes = [ctypes.c_int32, _dp, _dp, ctypes.c_double, ctypes.c_int64, ctypes.c_int64,
                                      ctypes.POINTER(_CParams), ctypes.c_int64, _dp]
         L.or_step_record.restype = ctypes.c_int
+        L.or_dumbbell_coords.argtypes = [ctypes.c_int32, _dp, _dp, _dp]
+        L.or_msd.argtypes = [ctypes.c_int32, ctypes.c_int32, _dp, _dp]
+        L.or_msd.restype = ctypes.c_double
         _lib = L
     return _lib
 
@@ -146,3 +149,21 @@ def step_record(X, phi, t0, n_done, n_steps, p: Params, stride: int):
     if rc:
         raise MemoryError("or_step_record")
     return X, traj
+
+
+def dumbbell_coords(X):
+    """Eq. (6a), (6b), PAPER.md:87-91: X [2S][3] -> (R [S][3], N [S][3])."""
+    X, xp = _d(X)
+    S = X.shape[0] // 2
+    R = np.empty((S, 3), dtype=np.float64)
+    Nv = np.empty((S, 3), dtype=np.float64)
+    lib().or_dumbbell_coords(S, xp, R.ctypes.data_as(_dp), Nv.ctypes.data_as(_dp))
+    return R, Nv
+
+
+def msd(Rt, R0):
+    """Eq. (13), PAPER.md:189: Rt, R0 [W][S][3] -> <<R(t)^2>>."""
+    Rt, rp = _d(Rt)
+    R0, r0p = _d(R0)
+    assert Rt.shape == R0.shape and Rt.ndim == 3
+    return float(lib().or_msd(Rt.shape[0], Rt.shape[1], rp, r0p))

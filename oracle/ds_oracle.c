@@ -18,6 +18,8 @@
  *                        u_(alpha i) = sum_beta H_(alpha i)(beta j) F_(beta j), matrix free
  *   or_velocity          forces followed by the mobility apply
  *   or_step              explicit Euler / one-step Heun predictor-corrector
+ *   or_dumbbell_coords   Eq. (6a,b) PAPER.md:87-91  direction and geometric centre of every dumbbell
+ *   or_msd               Eq. (13)  PAPER.md:189     mean square displacement per particle over W realisations
  *
  * Readings of the paper used here:
  *   R2  Heun = explicit trapezoid: X* = X + dt V(X,t); X' = X + dt/2 (V(X,t) + V(X*,t+dt)).
@@ -220,4 +222,38 @@ int or_step_record(int32_t S, double *X, const double *phi, double t0, int64_t n
         }
     }
     return 0;
+}
+
+/* Dumbbell coordinates, Eq. (6a), (6b), 0-based (dumbbell s = spheres 2s, 2s+1):
+ *   N^s = (X_{2s+1} - X_{2s}) / |X_{2s+1} - X_{2s}|,   R^s = (X_{2s+1} + X_{2s}) / 2.
+ * X [2S][3] -> R [S][3], Nv [S][3].                                                          */
+void or_dumbbell_coords(int32_t S, const double *X, double *R, double *Nv) {
+    for (int32_t s = 0; s < S; ++s) {
+        const double *x1 = X + 6 * (size_t)s, *x2 = x1 + 3;
+        double d[3], len2 = 0.0;
+        for (int c = 0; c < 3; ++c) { d[c] = x2[c] - x1[c]; len2 += d[c] * d[c]; }
+        const double len = sqrt(len2);
+        for (int c = 0; c < 3; ++c) {
+            Nv[3 * (size_t)s + c] = d[c] / len;
+            R[3 * (size_t)s + c] = 0.5 * (x2[c] + x1[c]);
+        }
+    }
+}
+
+/* Mean square displacement per particle averaged over W initial conditions, Eq. (13):
+ *   <<R(t)^2>> = (1/W) sum_w (1/S) sum_s |R^s(t; w) - R^s(0; w)|^2.
+ * Rt, R0 [W][S][3] (geometric centres, Eq. 6b).  Plain nested sums in the order of the formula. */
+double or_msd(int32_t W, int32_t S, const double *Rt, const double *R0) {
+    double outer = 0.0;
+    for (int32_t w = 0; w < W; ++w) {
+        double inner = 0.0;
+        for (int32_t s = 0; s < S; ++s) {
+            const size_t k = 3 * ((size_t)w * S + s);
+            double q = 0.0;
+            for (int c = 0; c < 3; ++c) { const double d = Rt[k + c] - R0[k + c]; q += d * d; }
+            inner += q;
+        }
+        outer += inner / (double)S;
+    }
+    return outer / (double)W;
 }

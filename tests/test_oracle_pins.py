@@ -369,3 +369,58 @@ def test_step_bookkeeping_time_from_step_index():
     u4 = oracle.mobility_apply(X, F, 1.0, 1.0, RPY)
     oracle.set_threads(1)
     assert np.array_equal(u1, u4)
+
+
+# --------------------------------------------------------------------------------- observables, Eq. (6a,b), (13)
+def test_P11_dumbbell_coordinates_closed_forms():
+    """PAPER.md:87-91 Eq. (6a), (6b).  A dumbbell placed at centre R along unit vector n with length L has exactly
+    that centre and direction (the input generator places spheres at R -/+ (L/2) n); swapping the two
+    spheres flips N and keeps R; translating by d shifts R by d and keeps N; N has unit length."""
+    rng = np.random.default_rng(11)
+    S = 7
+    Rc = rng.uniform(-50, 50, (S, 3))
+    n = rng.standard_normal((S, 3)); n /= np.linalg.norm(n, axis=1, keepdims=True)
+    L = rng.uniform(8, 12, S)
+    X = np.empty((2 * S, 3)); X[0::2] = Rc - 0.5 * L[:, None] * n; X[1::2] = Rc + 0.5 * L[:, None] * n
+    R, N = oracle.dumbbell_coords(X)
+    np.testing.assert_allclose(R, Rc, rtol=0, atol=1e-13)
+    np.testing.assert_allclose(N, n, rtol=0, atol=1e-14)
+    np.testing.assert_allclose(np.linalg.norm(N, axis=1), 1.0, rtol=0, atol=1e-15)
+    Xs = X.copy(); Xs[0::2], Xs[1::2] = X[1::2], X[0::2]
+    R2, N2 = oracle.dumbbell_coords(Xs)
+    assert np.array_equal(R2, R) and np.array_equal(N2, -N)
+    d = np.array([3.0, -4.0, 12.0])
+    R3, N3 = oracle.dumbbell_coords(X + d)
+    np.testing.assert_allclose(R3 - R, np.broadcast_to(d, R.shape), rtol=0, atol=1e-13)
+    np.testing.assert_allclose(N3, N, rtol=0, atol=1e-14)
+
+
+def test_P12_msd_closed_forms():
+    """PAPER.md:189 Eq. (13).  (i) zero displacement -> 0; (ii) every centre moved by the same vector d -> |d|^2
+    (3-4-12 triangle: 169 exactly); (iii) W realisations moved by different d_w -> the mean of |d_w|^2;
+    (iv) one dumbbell of S moved by d -> |d|^2 / S; (v) brute force with numpy on random data."""
+    rng = np.random.default_rng(12)
+    W, S = 5, 9
+    R0 = rng.uniform(-30, 30, (W, S, 3))
+    assert oracle.msd(R0, R0) == 0.0
+    assert oracle.msd(R0 + np.array([3.0, 4.0, 12.0]), R0) == pytest.approx(169.0, rel=1e-14)
+    dw = rng.standard_normal((W, 1, 3))
+    assert oracle.msd(R0 + dw, R0) == pytest.approx(float(np.mean(np.sum(dw ** 2, axis=-1))), rel=1e-13)
+    Rt = R0.copy(); Rt[2, 4] += np.array([1.0, 2.0, 2.0])
+    assert oracle.msd(Rt, R0) == pytest.approx(9.0 / (S * W), rel=1e-13)
+    Rt = R0 + rng.standard_normal(R0.shape)
+    assert oracle.msd(Rt, R0) == pytest.approx(float(np.mean(np.sum((Rt - R0) ** 2, axis=-1))), rel=1e-13)
+
+
+def test_P13_isolated_dumbbell_has_no_msd():
+    """Scallop theorem / I^sigma = 0: the centre of an isolated deterministic dumbbell does not
+    move, so Eq. (13) of a one-dumbbell system stays at rounding level over a period, while its direction is constant."""
+    p = oracle.Params()
+    phi = np.array([0.7])
+    n = np.array([[0.3, -0.5, 0.8]]); n /= np.linalg.norm(n)
+    X0 = inputs.place_spheres(np.array([[1.0, 2.0, 3.0]]), n, phi)
+    R0, N0 = oracle.dumbbell_coords(X0)
+    X = oracle.step(X0, phi, 0.0, 0, 1000, p)
+    R, N = oracle.dumbbell_coords(X)
+    assert oracle.msd(R[None], R0[None]) < 1e-24
+    np.testing.assert_allclose(N, N0, rtol=0, atol=1e-12)
