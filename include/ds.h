@@ -122,6 +122,18 @@ int ds_batch_step(ds_system *s, int64_t n_steps);
  * right-hand side of Eq. (1a) the integrator uses; exported for tests and observables).        */
 int ds_velocity(ds_system *s, void *V);
 
+/* Observables (computed on the device from the FP64 state).
+ * ds_dumbbell_coords: direction and geometric centre of every dumbbell, Eq. (6a), (6b):
+ *   N^s = (X_{2s+1} - X_{2s}) / |X_{2s+1} - X_{2s}|,  R^s = (X_{2s+1} + X_{2s}) / 2;
+ *   R, Nv are [B][S][3] in user precision; either may be NULL.
+ * ds_msd_set_reference: R^s(0; w) := the current centres (call it after the discarded first period).
+ * ds_msd: mean square displacement per particle averaged over the W = n_batch systems, Eq. (13):
+ *   (1/W) sum_w (1/S) sum_s |R^s(t; w) - R^s(0; w)|^2, written as one double to *msd (host or device pointer);
+ *   DS_ERR_STATE without a reference.                                                             */
+int ds_dumbbell_coords(ds_system *s, void *R, void *Nv);
+int ds_msd_set_reference(ds_system *s);
+int ds_msd(ds_system *s, double *msd);
+
 /* Launch-shape override for tuning and tests: number of row tiles (CTAs) per system; 0 = library
  * heuristic.  Values below ceil(ceil(N/4)/512) or above ceil(N/4) are clamped; the step modes also
  * clamp to the SM count (their CTAs meet at a barrier every stage and must be co-resident).      */

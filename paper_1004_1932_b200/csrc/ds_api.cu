@@ -67,6 +67,8 @@ struct ds_system {
     int64_t launches = 0;
     // state
     double *X = nullptr, *phase = nullptr;
+    double *Rref = nullptr, *msd_part = nullptr, *msd_out = nullptr;   // Eq. (13): reference centres, partial sums, result
+    bool has_ref = false;
     void *xu = nullptr;                         // the positions in user precision [B][N][3] (host-buffer fast path)
     bool x_valid = false, xu_valid = false;     // which of X (FP64) / xu holds the current state (at least one does)
     void *units[2] = {nullptr, nullptr};        // beta-streams (mobility.cuh), ping-pong over the stages
@@ -452,7 +454,7 @@ int ds_destroy(ds_system *s) {
     if (!s) return DS_OK;
     cudaSetDevice(s->P.device);
     cudaStreamSynchronize(s->stream);
-    void *ptrs[] = {s->X, s->xu, s->phase, s->units[0], s->units[1], s->ll[0], s->ll[1], s->bar, s->Xcg, s->V1g, s->Fg, s->Lg,
+    void *ptrs[] = {s->X, s->xu, s->Rref, s->msd_part, s->msd_out, s->phase, s->units[0], s->units[1], s->ll[0], s->ll[1], s->bar, s->Xcg, s->V1g, s->Fg, s->Lg,
                     s->ap_units.p, s->st_a.p, s->st_b.p, s->st_c.p};
     for (void *q : ptrs) if (q) cudaFree(q);
     (void)cudaGetLastError();
@@ -543,6 +545,72 @@ int ds_forces(ds_system *s, void *F) {
     DS_TRY(s->P.precision == DS_F64 ? run_forces_out<double>(s, dF) : run_forces_out<float>(s, dF));
     if (!dev) {
         CU_TRY(cudaMemcpyAsync(F, dF, nb, cudaMemcpyDeviceToHost, s->stream));
+        CU_TRY(cudaStreamSynchronize(s->stream));
+    }
+    return DS_OK;
+}
+
+int ds_dumbbell_coords(ds_system *s, void *R, void *Nv) {
+    if (!s) return DS_ERR_NULL;
+    if (!R && !Nv) return DS_ERR_NULL;
+    if (!s->has_state) return DS_ERR_STATE;
+    DS_TRY(set_device(s));
+    DS_TRY(materialize_x(s));
+    const long long n_db = (long long)s->B * s->S;
+    const size_t nb = (size_t)n_db * 3 * elem_size(s);
+    int rdev = 1, ndev = 1;
+    if (R) DS_TRY(is_device_ptr(R, &rdev));
+    if (Nv) DS_TRY(is_device_ptr(Nv, &ndev));
+    void *dR = R, *dN = Nv;
+    if (R && !rdev) { DS_TRY(ensure(s->st_b, nb)); dR = s->st_b.p; }
+    if (Nv && !ndev) { DS_TRY(ensure(s->st_c, nb)); dN = s->st_c.p; }
+    const unsigned grid = (unsigned)((n_db + 127) / 128);
+    if (s->P.precision == DS_F64)
+        ds::coords_kernel<double><<<grid, 128, 0, s->stream>>>(s->X, n_db, (double *)dR, (double *)dN, nullptr);
+    else
+        ds::coords_kernel<float><<<grid, 128, 0, s->stream>>>(s->X, n_db, (float *)dR, (float *)dN, nullptr);
+    CU_TRY(cudaGetLastError());
+    s->launches += 1;
+    if (R && !rdev) CU_TRY(cudaMemcpyAsync(R, dR, nb, cudaMemcpyDeviceToHost, s->stream));
+    if (Nv && !ndev) CU_TRY(cudaMemcpyAsync(Nv, dN, nb, cudaMemcpyDeviceToHost, s->stream));
+    if ((R && !rdev) || (Nv && !ndev)) CU_TRY(cudaStreamSynchronize(s->stream));
+    return DS_OK;
+}
+
+int ds_msd_set_reference(ds_system *s) {
+    if (!s) return DS_ERR_NULL;
+    if (!s->has_state) return DS_ERR_STATE;
+    DS_TRY(set_device(s));
+    DS_TRY(materialize_x(s));
+    const long long n_db = (long long)s->B * s->S;
+    if (!s->Rref) {
+        const int n_chunk = (s->S + 255) / 256;
+        CU_TRY(cudaMalloc((void **)&s->Rref, (size_t)n_db * 3 * sizeof(double)));
+        CU_TRY(cudaMalloc((void **)&s->msd_part, (size_t)s->B * n_chunk * sizeof(double)));
+        CU_TRY(cudaMalloc((void **)&s->msd_out, sizeof(double)));
+    }
+    ds::coords_kernel<double><<<(unsigned)((n_db + 127) / 128), 128, 0, s->stream>>>(s->X, n_db, nullptr, nullptr, s->Rref);
+    CU_TRY(cudaGetLastError());
+    s->launches += 1;
+    s->has_ref = true;
+    return DS_OK;
+}
+
+int ds_msd(ds_system *s, double *msd) {
+    if (!s || !msd) return DS_ERR_NULL;
+    if (!s->has_state || !s->has_ref) return DS_ERR_STATE;
+    DS_TRY(set_device(s));
+    DS_TRY(materialize_x(s));
+    int dev = 0;
+    DS_TRY(is_device_ptr(msd, &dev));
+    const int n_chunk = (s->S + 255) / 256;
+    ds::msd_partial_kernel<<<dim3((unsigned)n_chunk, (unsigned)s->B), 256, 0, s->stream>>>(s->X, s->Rref, s->S, s->msd_part);
+    CU_TRY(cudaGetLastError());
+    ds::msd_final_kernel<<<1, 256, 0, s->stream>>>(s->msd_part, s->B, s->S, n_chunk, dev ? msd : s->msd_out);
+    CU_TRY(cudaGetLastError());
+    s->launches += 2;
+    if (!dev) {
+        CU_TRY(cudaMemcpyAsync(msd, s->msd_out, sizeof(double), cudaMemcpyDeviceToHost, s->stream));
         CU_TRY(cudaStreamSynchronize(s->stream));
     }
     return DS_OK;

@@ -80,3 +80,69 @@ template <typename T> __global__ void state_out_kernel(const double *X, void *ou
 }
 
 }  // namespace ds
+
+namespace ds {
+
+// ---------------------------------------------------------------------------------------------
+// Observables.  Dumbbell coordinates, Eq. (6a), (6b), from the FP64 state:
+//   N^s = (X_{2s+1} - X_{2s}) / |X_{2s+1} - X_{2s}|,   R^s = (X_{2s+1} + X_{2s}) / 2.
+// One thread per dumbbell.  outR / outN in user precision (either may be NULL); Rref (FP64, may be NULL) receives
+// the centres as the reference R(0; w) of Eq. (13).
+template <typename T>
+__global__ void coords_kernel(const double *__restrict__ X, long long n_db, T *outR, T *outN, double *Rref) {
+    const long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n_db) return;
+    const double *x1 = X + 6 * s, *x2 = x1 + 3;
+    double d[3], len2 = 0.0;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { d[c] = x2[c] - x1[c]; len2 += d[c] * d[c]; }
+    const double len = sqrt(len2);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const double r = 0.5 * (x2[c] + x1[c]);
+        if (outR) outR[3 * s + c] = (T)r;
+        if (outN) outN[3 * s + c] = (T)(d[c] / len);
+        if (Rref) Rref[3 * s + c] = r;
+    }
+}
+
+// Eq. (13), first pass: block (chunk, w) adds |R^s(t; w) - R^s(0; w)|^2 over its <= 256 dumbbells
+// (shared-memory tree, fixed order) -> partial[w][chunk].
+__global__ void __launch_bounds__(256) msd_partial_kernel(const double *__restrict__ X, const double *__restrict__ Rref, int S,
+                                                          double *partial) {
+    __shared__ double sh[256];
+    const int w = blockIdx.y, s = blockIdx.x * 256 + threadIdx.x;
+    double q = 0.0;
+    if (s < S) {
+        const size_t k = (size_t)w * S + s;
+        const double *x1 = X + 6 * k, *x2 = x1 + 3, *r0 = Rref + 3 * k;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { const double d = 0.5 * (x2[c] + x1[c]) - r0[c]; q += d * d; }
+    }
+    sh[threadIdx.x] = q;
+    __syncthreads();
+    for (int h = 128; h > 0; h >>= 1) {
+        if (threadIdx.x < h) sh[threadIdx.x] += sh[threadIdx.x + h];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) partial[(size_t)w * gridDim.x + blockIdx.x] = sh[0];
+}
+// second pass (one block): (1/W) sum_w (1/S) sum_chunks partial[w][chunk], fixed order.
+__global__ void __launch_bounds__(256) msd_final_kernel(const double *__restrict__ partial, int W, int S, int n_chunk, double *out) {
+    __shared__ double sh[256];
+    double acc = 0.0;
+    for (int w = threadIdx.x; w < W; w += 256) {
+        double inner = 0.0;
+        for (int c = 0; c < n_chunk; ++c) inner += partial[(size_t)w * n_chunk + c];
+        acc += inner / (double)S;
+    }
+    sh[threadIdx.x] = acc;
+    __syncthreads();
+    for (int h = 128; h > 0; h >>= 1) {
+        if (threadIdx.x < h) sh[threadIdx.x] += sh[threadIdx.x + h];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *out = sh[0] / (double)W;
+}
+
+}  // namespace ds

@@ -22,7 +22,7 @@ ERR_INVALID_PARAM, ERR_NULL, ERR_CUDA, ERR_STATE, ERR_NO_DEVICE, ERR_ALLOC = -1,
 
 # every symbol include/ds.h declares (tests check that the built library exports all of them)
 SYMBOLS = ["ds_create", "ds_destroy", "ds_set_stream", "ds_set_state", "ds_get_state", "ds_forces",
-           "ds_mobility_apply", "ds_step", "ds_batch_step", "ds_velocity", "ds_set_tuning", "ds_set_probe", "ds_launch_count",
+           "ds_mobility_apply", "ds_step", "ds_batch_step", "ds_velocity", "ds_dumbbell_coords", "ds_msd_set_reference", "ds_msd", "ds_set_tuning", "ds_set_probe", "ds_launch_count",
            "ds_peak_probe", "ds_strerror", "ds_last_cuda_error", "ds_version"]
 
 
@@ -64,6 +64,9 @@ def lib():
         L.ds_step.argtypes = [vp, i64]
         L.ds_batch_step.argtypes = [vp, i64]
         L.ds_velocity.argtypes = [vp, vp]
+        L.ds_dumbbell_coords.argtypes = [vp, vp, vp]
+        L.ds_msd_set_reference.argtypes = [vp]
+        L.ds_msd.argtypes = [vp, ctypes.POINTER(dbl)]
         L.ds_set_tuning.argtypes = [vp, i32]
         L.ds_set_probe.argtypes = [vp, vp]
         L.ds_launch_count.argtypes = [vp]
@@ -155,6 +158,17 @@ class System:
 
     def velocity(self, V):
         _check(lib().ds_velocity(self._h, _ptr(V)), "ds_velocity")
+
+    def dumbbell_coords(self, R=None, Nv=None):
+        _check(lib().ds_dumbbell_coords(self._h, _ptr(R), _ptr(Nv)), "ds_dumbbell_coords")
+
+    def msd_set_reference(self):
+        _check(lib().ds_msd_set_reference(self._h), "ds_msd_set_reference")
+
+    def msd(self):
+        v = ctypes.c_double()
+        _check(lib().ds_msd(self._h, ctypes.byref(v)), "ds_msd")
+        return v.value
 
     def mobility_apply(self, pos, F, u, n):
         _check(lib().ds_mobility_apply(self._h, _ptr(pos), _ptr(F), _ptr(u), int(n)), "ds_mobility_apply")

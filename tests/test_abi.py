@@ -53,7 +53,8 @@ def test_null_and_invalid_arguments_are_rejected_before_any_device_work():
     for fn, args in [(L.ds_set_state, (None, None, None, 0.0)), (L.ds_get_state, (None, None, None)),
                      (L.ds_forces, (None, None)), (L.ds_mobility_apply, (None, None, None, None, 4)),
                      (L.ds_step, (None, 1)), (L.ds_batch_step, (None, 1)), (L.ds_velocity, (None, None)),
-                     (L.ds_set_tuning, (None, 0)), (L.ds_set_stream, (None, None))]:
+                     (L.ds_set_tuning, (None, 0)), (L.ds_set_stream, (None, None)),
+                     (L.ds_dumbbell_coords, (None, None, None)), (L.ds_msd_set_reference, (None,)), (L.ds_msd, (None, None))]:
         assert fn(*args) == ds.ERR_NULL
     assert L.ds_destroy(None) == ds.OK
     assert L.ds_launch_count(None) == 0

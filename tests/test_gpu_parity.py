@@ -391,3 +391,58 @@ def test_host_buffers_state_path_matches_device_buffers(precision):
     assert np.array_equal(res[True][4], res[True][5])
     Xo = oracle.step(X0[0].astype(np.float64), ph[0], 0.2, 0, 25, p)
     assert np.abs(res[True][4][0] - Xo).max() <= (1e-4 if precision == ds.F32 else 1e-10) * ELL
+
+
+# --------------------------------------------------------------------------------- observables, Eq. (6a,b), (13)
+@pytest.mark.parametrize("precision", [ds.F32, ds.F64])
+def test_observables_parity_batch(precision):
+    """Dumbbell coordinates Eq. (6a,b) and the mean square displacement Eq. (13) over W = B systems, computed on the
+    device from the FP64 state, against the oracle run on the same systems; reference set after 60 steps (the paper
+    discards the settling transient), host and device output buffers."""
+    w = inputs.config5(B=5, S=300)          # S spans two 256-dumbbell chunks of the reduction
+    s, p = make_system(w, precision)
+    X0 = rounded(w, precision)
+    with s:
+        with pytest.raises(ds.DsError):
+            s.msd_set_reference()                        # no state yet
+        s.set_state(dev(X0, precision), torch.as_tensor(w.phase, device="cuda"))
+        with pytest.raises(ds.DsError) as e:
+            s.msd()
+        assert e.value.code == ds.ERR_STATE               # no reference yet
+        s.batch_step(60)
+        s.msd_set_reference()
+        assert s.msd() == 0.0
+        s.batch_step(240)
+        msd_gpu = s.msd()
+        R = torch.empty((w.B, w.S, 3), dtype=TDT[precision], device="cuda")
+        Nh = np.empty((w.B, w.S, 3), dtype=NPDT[precision])
+        s.dumbbell_coords(R, Nh)
+        torch.cuda.synchronize()
+    Rref, Rt, Nt = [], [], []
+    for b in range(w.B):
+        Xa = oracle.step(X0[b], w.phase[b], 0.0, 0, 60, p)
+        Xb = oracle.step(Xa, w.phase[b], 0.0, 60, 240, p)
+        Rref.append(oracle.dumbbell_coords(Xa)[0])
+        r, n = oracle.dumbbell_coords(Xb)
+        Rt.append(r); Nt.append(n)
+    msd_or = oracle.msd(np.stack(Rt), np.stack(Rref))
+    tol_x = (1e-4 if precision == ds.F32 else 1e-10) * ELL
+    assert np.abs(R.cpu().numpy().astype(np.float64) - np.stack(Rt)).max() <= tol_x
+    assert np.abs(Nh.astype(np.float64) - np.stack(Nt)).max() <= tol_x / ELL * 10
+    # the displacements themselves are ~1e-2 a over 0.24 T: compare Eq. (13) through the per-dumbbell error bound
+    disp = np.sqrt(msd_or)
+    assert abs(np.sqrt(msd_gpu) - disp) <= (2e-5 if precision == ds.F32 else 1e-9)
+    assert msd_gpu > 0.0
+
+
+def test_msd_closed_form_on_gpu():
+    """Eq. (13) on the device against its closed form: every system translated rigidly by its own vector d_w gives
+    the mean of |d_w|^2 (no dynamics involved: set_state, reference, set_state again)."""
+    w = inputs.config5(B=3, S=40)
+    dw = np.array([[3.0, 4.0, 12.0], [1.0, 2.0, 2.0], [0.0, 0.0, 0.5]])
+    s, _ = make_system(w, ds.F64)
+    with s:
+        s.set_state(dev(w.pos, ds.F64), torch.as_tensor(w.phase, device="cuda"))
+        s.msd_set_reference()
+        s.set_state(dev(w.pos + dw[:, None, :], ds.F64), torch.as_tensor(w.phase, device="cuda"))
+        np.testing.assert_allclose(s.msd(), np.mean(np.sum(dw ** 2, axis=1)), rtol=1e-12)
