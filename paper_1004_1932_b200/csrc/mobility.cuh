@@ -551,9 +551,15 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
                         const T *rp = reinterpret_cast<const T *>(A.raw_pos) + 3 * (r0 + il);
                         x = __ldg(rp); y = __ldg(rp + 1); z = __ldg(rp + 2);
                     } else {
-                        x = __ldcg(units + unit_index<T>(r0 + il, 0));
-                        y = __ldcg(units + unit_index<T>(r0 + il, 1));
-                        z = __ldcg(units + unit_index<T>(r0 + il, 2));
+                        // local mode keeps the stream in shared memory only (r0 = 0 there)
+                        if (local) {
+                            const T *us = reinterpret_cast<const T *>(smem_raw);
+                            x = us[unit_index<T>(il, 0)]; y = us[unit_index<T>(il, 1)]; z = us[unit_index<T>(il, 2)];
+                        } else {
+                            x = __ldcg(units + unit_index<T>(r0 + il, 0));
+                            y = __ldcg(units + unit_index<T>(r0 + il, 1));
+                            z = __ldcg(units + unit_index<T>(r0 + il, 2));
+                        }
                     }
                 }
             }

@@ -322,9 +322,19 @@ def test_step_stream_larger_than_shared_memory():
     """N = 16384 (FP32): the stage input (384 KB) does not fit a CTA's shared memory, so the step kernel streams it
     through the TMA ring and keeps the blocking barrier; 2 Heun steps against the oracle."""
     w = inputs.config5(B=1, S=8192)
-    Xg, X0, p = gpu_steps(w, ds.F32, 2)
-    Xo = oracle.step(X0[0], w.phase[0], 0.0, 0, 2, p)
-    assert np.abs(Xg[0] - Xo).max() <= 1e-4 * ELL
+    s, p = make_system(w, ds.F32)
+    X0 = rounded(w, ds.F32)
+    with s:
+        s.set_state(dev(X0, ds.F32), torch.as_tensor(w.phase, device="cuda"), t0=0.13)
+        out = torch.empty((1, w.N, 3), dtype=torch.float32, device="cuda")
+        V = torch.empty_like(out)
+        s.velocity(V)            # at the state just set: the FP64 state is exactly the float32 input widened
+        s.step(2)
+        s.get_state(out)
+        torch.cuda.synchronize()
+    assert rel_l2(V.cpu().numpy()[0].astype(np.float64), oracle.velocity(X0[0], w.phase[0], 0.13, p)) <= TOL[ds.F32]
+    Xo = oracle.step(X0[0], w.phase[0], 0.13, 0, 2, p)
+    assert np.abs(out.cpu().numpy()[0].astype(np.float64) - Xo).max() <= 1e-4 * ELL
 
 
 def test_batch_more_systems_than_sms():
@@ -446,3 +456,24 @@ def test_msd_closed_form_on_gpu():
         s.msd_set_reference()
         s.set_state(dev(w.pos + dw[:, None, :], ds.F64), torch.as_tensor(w.phase, device="cuda"))
         np.testing.assert_allclose(s.msd(), np.mean(np.sum(dw ** 2, axis=1)), rtol=1e-12)
+
+
+@pytest.mark.parametrize("n_tiles", [1, 2])
+def test_step_state_in_global_memory(n_tiles):
+    """Row tiles too large for the shared-memory state (here forced: N = 1600 in 1 or 2 CTAs, 800+ rows each): the
+    per-row state lives in the library's global arrays instead; same results."""
+    w = inputs.config5(B=1, S=800)
+    s, p = make_system(w, ds.F64)
+    X0 = rounded(w, ds.F64)
+    with s:
+        s.set_tuning(n_tiles)
+        s.set_state(np.ascontiguousarray(X0), np.ascontiguousarray(w.phase), t0=0.05)     # host buffers: starts from the user-precision image
+        s.step(12)
+        out = torch.empty((1, w.N, 3), dtype=torch.float64, device="cuda")
+        s.get_state(out)
+        V = torch.empty_like(out)
+        s.velocity(V)
+        torch.cuda.synchronize()
+    Xo = oracle.step(X0[0], w.phase[0], 0.05, 0, 12, p)
+    assert np.abs(out.cpu().numpy()[0] - Xo).max() <= 1e-10 * ELL
+    assert rel_l2(V.cpu().numpy()[0], oracle.velocity(Xo, w.phase[0], 0.05 + 12 * p.dt, p)) <= 1e-9
