@@ -477,3 +477,25 @@ def test_step_state_in_global_memory(n_tiles):
     Xo = oracle.step(X0[0], w.phase[0], 0.05, 0, 12, p)
     assert np.abs(out.cpu().numpy()[0] - Xo).max() <= 1e-10 * ELL
     assert rel_l2(V.cpu().numpy()[0], oracle.velocity(Xo, w.phase[0], 0.05 + 12 * p.dt, p)) <= 1e-9
+
+
+@pytest.mark.parametrize("n_tiles", [0, 100])
+def test_batch_in_several_launch_groups(n_tiles):
+    """B = 5 systems of N = 1024: with the library's shape all five share one launch (29 CTAs each); with 100 CTAs per
+    system only one system is co-resident at a time, so the call runs five launches one after the other."""
+    w = inputs.config5(B=5, S=512)
+    s, p = make_system(w, ds.F64)
+    X0 = rounded(w, ds.F64)
+    with s:
+        s.set_tuning(n_tiles)
+        s.set_state(dev(X0, ds.F64), torch.as_tensor(w.phase, device="cuda"))
+        l0 = s.launch_count()
+        s.batch_step(40)
+        n_launch = s.launch_count() - l0
+        out = torch.empty((w.B, w.N, 3), dtype=torch.float64, device="cuda")
+        s.get_state(out)
+        torch.cuda.synchronize()
+    assert n_launch == (5 if n_tiles == 100 else 1)
+    for b in (0, 3, 4):
+        Xo = oracle.step(X0[b], w.phase[b], 0.0, 0, 40, p)
+        assert np.abs(out.cpu().numpy()[b] - Xo).max() <= 1e-10 * ELL
