@@ -20,7 +20,8 @@ EULER, HEUN = 0, 1
 class _CParams(ctypes.Structure):
     _fields_ = [("a", ctypes.c_double), ("eta", ctypes.c_double), ("ell", ctypes.c_double),
                 ("lam", ctypes.c_double), ("omega", ctypes.c_double), ("k0", ctypes.c_double),
-                ("dt", ctypes.c_double), ("tensor", ctypes.c_int32), ("integrator", ctypes.c_int32)]
+                ("dt", ctypes.c_double), ("tensor", ctypes.c_int32), ("integrator", ctypes.c_int32),
+                ("kT", ctypes.c_double), ("seed", ctypes.c_uint64), ("system", ctypes.c_int32)]
 
 
 @dataclass
@@ -35,10 +36,13 @@ class Params:
     dt: float = 1e-3
     tensor: int = RPY
     integrator: int = HEUN
+    kT: float = 0.0        # thermal energy of Eq. (1a); 0 = the deterministic limit the paper simulates
+    seed: int = 0          # key of the counter-based generator
+    system: int = 0        # index w of the realisation (enters the generator's counter)
 
     def c(self) -> _CParams:
         return _CParams(self.a, self.eta, self.ell, self.lam, self.omega, self.k0, self.dt,
-                        int(self.tensor), int(self.integrator))
+                        int(self.tensor), int(self.integrator), float(self.kT), int(self.seed), int(self.system))
 
 
 _lib = None
@@ -63,6 +67,9 @@ def lib():
         L.or_step_record.argtypes = [ctypes.c_int32, _dp, _dp, ctypes.c_double, ctypes.c_int64, ctypes.c_int64,
                                      ctypes.POINTER(_CParams), ctypes.c_int64, _dp]
         L.or_step_record.restype = ctypes.c_int
+        L.or_philox4x32_10.argtypes = [ctypes.POINTER(ctypes.c_uint32)] * 3
+        L.or_noise_normal.argtypes = [ctypes.c_uint64, ctypes.c_int64, ctypes.c_int32, ctypes.c_int64]
+        L.or_noise_normal.restype = ctypes.c_double
         L.or_dumbbell_coords.argtypes = [ctypes.c_int32, _dp, _dp, _dp]
         L.or_msd.argtypes = [ctypes.c_int32, ctypes.c_int32, _dp, _dp]
         L.or_msd.restype = ctypes.c_double
@@ -167,3 +174,17 @@ def msd(Rt, R0):
     R0, r0p = _d(R0)
     assert Rt.shape == R0.shape and Rt.ndim == 3
     return float(lib().or_msd(Rt.shape[0], Rt.shape[1], rp, r0p))
+
+
+def philox4x32_10(ctr, key):
+    """The generator behind the Brownian increments: counter [4] uint32, key [2] uint32 -> [4] uint32."""
+    c = (ctypes.c_uint32 * 4)(*[int(v) & 0xffffffff for v in ctr])
+    k = (ctypes.c_uint32 * 2)(*[int(v) & 0xffffffff for v in key])
+    o = (ctypes.c_uint32 * 4)()
+    lib().or_philox4x32_10(c, k, o)
+    return [int(v) for v in o]
+
+
+def noise_normal(seed, n, system, element):
+    """z ~ N(0,1) of step n, realisation `system`, state element 3 alpha + i (Eq. 1b, 1c)."""
+    return float(lib().or_noise_normal(int(seed), int(n), int(system), int(element)))

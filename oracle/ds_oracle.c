@@ -18,6 +18,7 @@
  *                        u_(alpha i) = sum_beta H_(alpha i)(beta j) F_(beta j), matrix free
  *   or_velocity          forces followed by the mobility apply
  *   or_step              explicit Euler / one-step Heun predictor-corrector
+ *   or_noise_normal      Eq. (1a-c), additive approximation of PAPER.md:240: the Gaussian increments (Philox4x32-10)
  *   or_dumbbell_coords   Eq. (6a,b) PAPER.md:87-91  direction and geometric centre of every dumbbell
  *   or_msd               Eq. (13)  PAPER.md:189     mean square displacement per particle over W realisations
  *
@@ -67,6 +68,9 @@ typedef struct {
     double dt;     /* time step */
     int32_t tensor;     /* OR_OSEEN: first line of (3b) only; OR_RPY: both */
     int32_t integrator; /* OR_EULER or OR_HEUN                           */
+    double kT;          /* thermal energy k_B T of Eq. (1a); 0 = deterministic limit */
+    uint64_t seed;      /* key of the counter-based generator behind xi(t)                */
+    int32_t system;     /* index w of this realisation in a batch (enters the counter)   */
 } or_params;
 
 static int g_threads = 1;
@@ -185,22 +189,56 @@ void or_velocity(int32_t S, const double *X, const double *phi, double t, const 
 
 /* n_steps explicit steps from step index n_done (reading R2).
  * t_n = t0 + n dt (R7).  X is updated in place.  Returns 0, or -1 if out of memory.       */
+/* Brownian term, Eq. (1a)-(2) in the additive approximation the paper advocates:
+ * "a simple additive noise with a constant matrix C ... as the off-diagonal terms in Eq. (3) are negligible", i.e.
+ * 2H = C C^T with H reduced to its diagonal (3a): C = sqrt(2 / (6 pi mu a)) 1.  Integrated over one step the term
+ * (k_B T)^(1/2) C xi(t) becomes dW_(alpha i) = sqrt(2 k_B T dt / (6 pi mu a)) z, z ~ N(0,1) independent per sphere,
+ * component and step (Eq. 1b, 1c).  z comes from a counter-based generator so that any implementation can draw
+ * the same numbers: Philox4x32-10 (Salmon et al., SC'11) with counter (n lo, n hi, 3 alpha + i, w), key (seed lo,
+ * seed hi); its first two words u1, u2 -> Box-Muller z = sqrt(-2 ln U1) cos(2 pi U2), U = (u + 0.5) / 2^32.       */
+void or_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3], k0 = key[0], k1 = key[1];
+    for (int r = 0; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0, n1 = (uint32_t)p1;
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1, n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+double or_noise_normal(uint64_t seed, int64_t n, int32_t system, int64_t element) {
+    const uint32_t ctr[4] = {(uint32_t)((uint64_t)n & 0xffffffffu), (uint32_t)((uint64_t)n >> 32), (uint32_t)element,
+                             (uint32_t)system};
+    const uint32_t key[2] = {(uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32)};
+    uint32_t w[4];
+    or_philox4x32_10(ctr, key, w);
+    const double U1 = ((double)w[0] + 0.5) / 4294967296.0, U2 = ((double)w[1] + 0.5) / 4294967296.0;
+    return sqrt(-2.0 * log(U1)) * cos(6.283185307179586476925286766559 * U2);
+}
+
+/* Explicit Euler / one-step Heun predictor-corrector.  With k_B T > 0 the same increment dW enters the
+ * predictor and the corrector (stochastic Heun for additive noise: "can easily incorporate additive noise").        */
 int or_step(int32_t S, double *X, const double *phi, double t0, int64_t n_done, int64_t n_steps,
             const or_params *p) {
     size_t M = 6 * (size_t)S;
-    double *buf = (double *)malloc(4 * M * sizeof(double));
+    double *buf = (double *)malloc(5 * M * sizeof(double));
     if (!buf) return -1;
-    double *V1 = buf, *V2 = buf + M, *Xp = buf + 2 * M, *Fw = buf + 3 * M;
+    double *V1 = buf, *V2 = buf + M, *Xp = buf + 2 * M, *Fw = buf + 3 * M, *dW = buf + 4 * M;
+    const double pi = 3.14159265358979323846264338327950288;
+    const double amp = sqrt(2.0 * p->kT * p->dt / (6.0 * pi * p->eta * p->a));
     for (int64_t n = n_done; n < n_done + n_steps; ++n) {
         double t = t0 + (double)n * p->dt;
+        for (size_t k = 0; k < M; ++k) dW[k] = p->kT > 0.0 ? amp * or_noise_normal(p->seed, n, p->system, (int64_t)k) : 0.0;
         or_velocity(S, X, phi, t, p, V1, Fw);
         if (p->integrator == OR_EULER) {
-            for (size_t k = 0; k < M; ++k) X[k] = X[k] + p->dt * V1[k];
+            for (size_t k = 0; k < M; ++k) X[k] = X[k] + p->dt * V1[k] + dW[k];
         } else {
             double t1 = t0 + (double)(n + 1) * p->dt;
-            for (size_t k = 0; k < M; ++k) Xp[k] = X[k] + p->dt * V1[k];
+            for (size_t k = 0; k < M; ++k) Xp[k] = X[k] + p->dt * V1[k] + dW[k];
             or_velocity(S, Xp, phi, t1, p, V2, Fw);
-            for (size_t k = 0; k < M; ++k) X[k] = X[k] + 0.5 * p->dt * (V1[k] + V2[k]);
+            for (size_t k = 0; k < M; ++k) X[k] = X[k] + 0.5 * p->dt * (V1[k] + V2[k]) + dW[k];
         }
     }
     free(buf);

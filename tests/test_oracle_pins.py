@@ -424,3 +424,74 @@ def test_P13_isolated_dumbbell_has_no_msd():
     R, N = oracle.dumbbell_coords(X)
     assert oracle.msd(R[None], R0[None]) < 1e-24
     np.testing.assert_allclose(N, N0, rtol=0, atol=1e-12)
+
+
+# --------------------------------------------------------------------------------- Brownian term, additive approximation
+def test_P14_philox_known_answers():
+    """The generator is Philox4x32-10 as published: tests/golden/philox4x32_10_kat.txt (Salmon et al., SC'11)."""
+    rows = [l.split() for l in open(os.path.join(GOLD, "philox4x32_10_kat.txt")) if l.strip() and not l.startswith("#")]
+    assert len(rows) == 3
+    for r in rows:
+        v = [int(x, 16) for x in r]
+        assert oracle.philox4x32_10(v[0:4], v[4:6]) == v[6:10]
+
+
+def test_P15_increments_are_standard_normal_and_independent():
+    """Eq. (1b), (1c): <xi> = 0, <xi xi'> = delta: unit variance, no correlation between steps, spheres /
+    components, realisations or seeds (counter-based draws: sample moments within 4 standard errors)."""
+    n = 40000
+    z = np.array([oracle.noise_normal(7, k, 0, 0) for k in range(n)])
+    ze = np.array([oracle.noise_normal(7, 0, 0, k) for k in range(n)])
+    zs = np.array([oracle.noise_normal(7, 0, k, 0) for k in range(n)])
+    z2 = np.array([oracle.noise_normal(8, k, 0, 0) for k in range(n)])
+    for v in (z, ze, zs, z2):
+        assert abs(v.mean()) < 4 / np.sqrt(n)
+        assert abs(v.var() - 1.0) < 4 * np.sqrt(2.0 / n)
+        assert abs(np.mean(v ** 4) - 3.0) < 4 * np.sqrt(96.0 / n)
+        assert abs(np.mean(v[1:] * v[:-1])) < 4 / np.sqrt(n)
+    for a, b in ((z, ze), (z, zs), (z, z2), (ze, zs)):
+        assert abs(np.mean(a * b)) < 4 / np.sqrt(n)
+    assert oracle.noise_normal(7, 5, 2, 11) == oracle.noise_normal(7, 5, 2, 11)      # a pure function of its counter
+
+
+def test_P16_isolated_dumbbell_centre_is_the_sum_of_its_increments():
+    """Additive noise, with the shared-increment Heun step: for an isolated dumbbell the
+    deterministic velocities of the two spheres cancel (I^sigma = 0), so the centre moves by exactly
+    (dW_1 + dW_2)/2 per step, dW = sqrt(2 kT dt / (6 pi eta a)) z.  Checked against the generator's own draws, and the
+    ensemble mean square displacement against 6 D_R t with D_R = kT / (12 pi eta a)."""
+    kT, seed, nst = 0.05, 99, 60
+    p = oracle.Params(kT=kT, seed=seed, system=3)
+    phi = np.array([1.1])
+    n = np.array([[0.2, 0.9, -0.4]]); n /= np.linalg.norm(n)
+    X0 = inputs.place_spheres(np.array([[0.0, 0.0, 0.0]]), n, phi)
+    X = oracle.step(X0, phi, 0.0, 0, nst, p)
+    amp = np.sqrt(2 * kT * p.dt / (6 * np.pi * p.eta * p.a))
+    expect = np.zeros(3)
+    for m in range(nst):
+        for c in range(3):
+            expect[c] += 0.5 * amp * (oracle.noise_normal(seed, m, 3, c) + oracle.noise_normal(seed, m, 3, 3 + c))
+    R0, _ = oracle.dumbbell_coords(X0); R, _ = oracle.dumbbell_coords(X)
+    np.testing.assert_allclose((R - R0)[0], expect, rtol=0, atol=1e-13)
+    # ensemble: W realisations (system index w), MSD of the centre = 3 * (2 D_R) t = kT t / (2 pi eta a)
+    W = 400
+    disp2 = []
+    for w_ in range(W):
+        Xw = oracle.step(X0, phi, 0.0, 0, nst, oracle.Params(kT=kT, seed=seed, system=w_))
+        disp2.append(np.sum((oracle.dumbbell_coords(Xw)[0] - R0) ** 2))
+    theory = kT * nst * p.dt / (2 * np.pi * p.eta * p.a)
+    assert abs(np.mean(disp2) / theory - 1.0) < 4 * np.sqrt(2.0 / (3 * W))
+
+
+def test_P17_zero_temperature_is_the_deterministic_path():
+    """kT = 0 is the deterministic limit: bit-identical to a run that never heard of the noise term; a
+    different seed changes nothing then, and at kT > 0 Euler's first step is X + dt V + dW exactly."""
+    w = inputs.config1()
+    a = oracle.step(w.pos[0], w.phase[0], 0.0, 0, 50, oracle.Params())
+    b = oracle.step(w.pos[0], w.phase[0], 0.0, 0, 50, oracle.Params(kT=0.0, seed=1234, system=9))
+    assert np.array_equal(a, b)
+    pe = oracle.Params(integrator=oracle.EULER, kT=0.3, seed=5)
+    V = oracle.velocity(w.pos[0], w.phase[0], 0.0, pe)
+    amp = np.sqrt(2 * pe.kT * pe.dt / (6 * np.pi))
+    dW = amp * np.array([oracle.noise_normal(5, 0, 0, k) for k in range(w.N * 3)]).reshape(w.N, 3)
+    X1 = oracle.step(w.pos[0], w.phase[0], 0.0, 0, 1, pe)
+    np.testing.assert_allclose(X1, w.pos[0] + pe.dt * V + dW, rtol=0, atol=1e-13)
