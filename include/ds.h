@@ -33,7 +33,8 @@
  *   applied for every r > 0, the paper has no overlap branch; its stated validity range is
  *   r > 2a), and finite inputs.
  *
- * The library draws no random numbers.
+ * The library keeps no random state: with kT > 0 the Brownian increments are a pure function of (seed, step, system,
+ * sphere, component).
  */
 #ifndef DS_H_
 #define DS_H_
@@ -75,11 +76,17 @@ typedef struct {
     double k0;           /* spring constant                        PAPER.md:65 Eq. (4)           */
     double dt;           /* time step                  */
     void *stream;        /* cudaStream_t the work is enqueued on; NULL = legacy default stream   */
+    double kT;           /* thermal energy k_B T of Eq. (1a); 0 = the deterministic limit
+                            the paper simulates.  > 0: additive Brownian increments
+                            dW = sqrt(2 kT dt / (6 pi eta a)) z per sphere, component and step, the constant-C
+                            approximation of PAPER.md:240; z from Philox4x32-10 keyed by `seed`, counter
+                            (step, state element, system)                                            */
+    uint64_t seed;       /* key of the generator (the library itself keeps no random state)        */
 } ds_params;
 
 /* Validate p, allocate the system's device buffers and build its CUDA graphs.
  * Rejects (DS_ERR_INVALID_PARAM): S < 1, B < 1, unknown enum values, non-positive or non-finite
- * a, eta, k0, dt, ell, negative omega, and ell <= 2a + |lambda|.               */
+ * a, eta, k0, dt, ell, negative omega, negative or non-finite kT, and ell <= 2a + |lambda|.               */
 int ds_create(const ds_params *p, ds_system **out);
 
 /* Free everything the system owns.  Synchronises the system's stream first.  NULL is a no-op. */

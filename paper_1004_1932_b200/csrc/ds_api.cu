@@ -253,6 +253,8 @@ void fill_constants(const ds_system *s, ds::RunArgs &A) {
     A.c2 = 2.0 * s->P.a * s->P.a;
     A.c1f = (float)A.c1; A.c2f = (float)A.c2;
     A.t0 = s->t0; A.dt = s->P.dt; A.ell = s->P.ell; A.lambda = s->P.lambda; A.omega = s->P.omega; A.k0 = s->P.k0;
+    A.noise_amp = s->P.kT > 0.0 ? sqrt(2.0 * s->P.kT * s->P.dt * A.self_mob) : 0.0;   // Eq. (1a) with 2H ~ 2/(6 pi mu a) = C C^T
+    A.seed = s->P.seed;
 }
 
 // RUN_VELOCITY (n_steps ignored) or RUN_STEP on the system's own state: one launch per group of
@@ -402,6 +404,7 @@ int ds_create(const ds_params *p, ds_system **out) {
     if (!isfinite(p->lambda) || !isfinite(p->omega) || p->omega < 0.0) return DS_ERR_INVALID_PARAM;
     if (!(p->ell > 2.0 * p->a + fabs(p->lambda))) return DS_ERR_INVALID_PARAM;
     if (p->n_batch > 65535) return DS_ERR_INVALID_PARAM;
+    if (!isfinite(p->kT) || p->kT < 0.0) return DS_ERR_INVALID_PARAM;
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { (void)cudaGetLastError(); return DS_ERR_NO_DEVICE; }

@@ -40,6 +40,7 @@
 
 #include <type_traits>
 
+#include "noise.cuh"
 #include "pack.cuh"
 
 namespace ds {
@@ -86,6 +87,8 @@ struct RunArgs {
     int from_user;            // 1: the launch starts from xu (ds_set_state with a host buffer left X stale)
     const double *phase;      // [B][S]
     double t0, dt, ell, lambda, omega, k0;
+    double noise_amp;         // sqrt(2 k_B T dt / (6 pi mu a)): Brownian increments (noise.cuh); 0 = deterministic
+    unsigned long long seed;
     // inter-CTA barrier: one monotonic arrival counter per system; this launch starts at bar_base
     unsigned long long *bar;
     unsigned long long bar_base;
@@ -802,12 +805,16 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
                     continue;
                 }
                 // predictor X* = X_n + dt V1;  corrector X_{n+1} = X_n + (dt/2)(V1 + V2);  Euler X_{n+1} = X_n + dt V
+                // with k_B T > 0 the same increment dW enters the predictor and the corrector (stochastic Heun for
+                // additive noise; "can easily incorporate additive noise")
                 const double cdt = corr ? 0.5 * A.dt : A.dt;
+                const long long nstep = A.n0 + (MODE == KM_HEUN ? (g >> 1) : g);
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
                     const int e = e0 + j;
                     const double w = corr ? v1[j] + v[j] : v[j];
-                    const double xn = xo[j] + cdt * w;
+                    double xn = xo[j] + cdt * w;
+                    if (A.noise_amp != 0.0) xn += A.noise_amp * noise_normal(A.seed, nstep, b, 3 * r0 + e);
                     if (pred) V1s[e] = v[j]; else Xs[e] = xn;
                     Xc[e] = xn;
                     if (XcT != nullptr) XcT[e] = (T)xn;

@@ -41,7 +41,7 @@ class Params(ctypes.Structure):
                 ("tensor", ctypes.c_int32), ("integrator", ctypes.c_int32), ("device", ctypes.c_int32),
                 ("a", ctypes.c_double), ("eta", ctypes.c_double), ("ell", ctypes.c_double),
                 ("lam", ctypes.c_double), ("omega", ctypes.c_double), ("k0", ctypes.c_double),
-                ("dt", ctypes.c_double), ("stream", ctypes.c_void_p)]
+                ("dt", ctypes.c_double), ("stream", ctypes.c_void_p), ("kT", ctypes.c_double), ("seed", ctypes.c_uint64)]
 
 
 _lib = None
@@ -116,11 +116,11 @@ class System:
     """Owner of one ds_system handle; method names and arguments follow include/ds.h."""
 
     def __init__(self, n_dumbbells, n_batch=1, precision=F64, tensor=RPY, integrator=HEUN, a=1.0, eta=1.0,
-                 ell=10.0, lam=2.0, omega=2.0 * np.pi, k0=1000.0, dt=1e-3, device=0, stream=None):
+                 ell=10.0, lam=2.0, omega=2.0 * np.pi, k0=1000.0, dt=1e-3, device=0, stream=None, kT=0.0, seed=0):
         self._h = ctypes.c_void_p()
         self.params = Params(int(n_dumbbells), int(n_batch), int(precision), int(tensor), int(integrator),
                              int(device), float(a), float(eta), float(ell), float(lam), float(omega),
-                             float(k0), float(dt), ctypes.c_void_p(stream) if stream else None)
+                             float(k0), float(dt), ctypes.c_void_p(stream) if stream else None, float(kT), int(seed))
         _check(lib().ds_create(ctypes.byref(self.params), ctypes.byref(self._h)), "ds_create")
         self.S, self.N, self.B = int(n_dumbbells), 2 * int(n_dumbbells), int(n_batch)
         self.precision = int(precision)

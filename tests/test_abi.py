@@ -40,14 +40,14 @@ def test_null_and_invalid_arguments_are_rejected_before_any_device_work():
     h = ctypes.c_void_p()
     assert L.ds_create(None, ctypes.byref(h)) == ds.ERR_NULL
     good = dict(n_dumbbells=4, n_batch=1, precision=ds.F64, tensor=ds.RPY, integrator=ds.HEUN, device=0,
-                a=1.0, eta=1.0, ell=10.0, lam=2.0, omega=6.28, k0=1000.0, dt=1e-3)
+                a=1.0, eta=1.0, ell=10.0, lam=2.0, omega=6.28, k0=1000.0, dt=1e-3, kT=0.0)
     bad = [dict(n_dumbbells=0), dict(n_batch=0), dict(precision=7), dict(tensor=-1), dict(integrator=2),
            dict(a=0.0), dict(eta=-1.0), dict(k0=0.0), dict(dt=float("nan")), dict(ell=4.0),   # ell <= 2a + lam
-           dict(lam=8.0), dict(lam=-8.0), dict(omega=-1.0), dict(dt=float("inf"))]
+           dict(lam=8.0), dict(lam=-8.0), dict(omega=-1.0), dict(dt=float("inf")), dict(kT=-1.0), dict(kT=float("nan"))]
     for change in bad:
         kw = dict(good, **change)
         p = ds.Params(kw["n_dumbbells"], kw["n_batch"], kw["precision"], kw["tensor"], kw["integrator"], kw["device"],
-                      kw["a"], kw["eta"], kw["ell"], kw["lam"], kw["omega"], kw["k0"], kw["dt"], None)
+                      kw["a"], kw["eta"], kw["ell"], kw["lam"], kw["omega"], kw["k0"], kw["dt"], None, kw["kT"], 0)
         assert L.ds_create(ctypes.byref(p), ctypes.byref(h)) == ds.ERR_INVALID_PARAM, change
         assert not h.value
     for fn, args in [(L.ds_set_state, (None, None, None, 0.0)), (L.ds_get_state, (None, None, None)),

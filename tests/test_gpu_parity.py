@@ -133,9 +133,10 @@ def make_system(w, precision, tensor=ds.RPY, integrator=ds.HEUN, **kw):
     sc = dict(w.scalars)
     sc.update(kw)
     s = ds.System(w.S, n_batch=w.B, precision=precision, tensor=tensor, integrator=integrator, a=sc["a"],
-                  eta=sc["eta"], ell=sc["ell"], lam=sc["lam"], omega=sc["omega"], k0=sc["k0"], dt=sc["dt"])
+                  eta=sc["eta"], ell=sc["ell"], lam=sc["lam"], omega=sc["omega"], k0=sc["k0"], dt=sc["dt"],
+                  kT=sc.get("kT", 0.0), seed=sc.get("seed", 0))
     return s, oracle.Params(a=sc["a"], eta=sc["eta"], ell=sc["ell"], lam=sc["lam"], omega=sc["omega"], k0=sc["k0"],
-                            dt=sc["dt"], tensor=tensor, integrator=integrator)
+                            dt=sc["dt"], tensor=tensor, integrator=integrator, kT=sc.get("kT", 0.0), seed=sc.get("seed", 0))
 
 
 def rounded(w, precision):
@@ -499,3 +500,40 @@ def test_batch_in_several_launch_groups(n_tiles):
     for b in (0, 3, 4):
         Xo = oracle.step(X0[b], w.phase[b], 0.0, 0, 40, p)
         assert np.abs(out.cpu().numpy()[b] - Xo).max() <= 1e-10 * ELL
+
+
+# --------------------------------------------------------------------------------- Brownian term (additive approximation)
+@pytest.mark.parametrize("integrator", [ds.EULER, ds.HEUN])
+@pytest.mark.parametrize("precision,tol", [(ds.F64, 1e-9), (ds.F32, 1e-4)])
+def test_step_with_additive_noise_matches_oracle(precision, tol, integrator):
+    """kT > 0 (Eq. (1a) in the constant-C approximation of PAPER.md:240): the device draws the same
+    Philox4x32-10 increments as the oracle (counter = step, element, system), so trajectories agree like the
+    deterministic ones do; 3 systems = 3 realisations w, several launch shapes, steps split over calls."""
+    import dataclasses
+    w = inputs.config5(B=3, S=96)
+    X0 = rounded(w, precision)
+    for n_tiles in (1, 6):
+        s, p = make_system(w, precision, integrator=integrator, kT=0.02, seed=0x1234567ABCDEF)
+        with s:
+            s.set_tuning(n_tiles)
+            s.set_state(dev(X0, precision), torch.as_tensor(w.phase, device="cuda"))
+            s.batch_step(37)
+            s.batch_step(63)
+            out = torch.empty((w.B, w.N, 3), dtype=TDT[precision], device="cuda")
+            s.get_state(out)
+            torch.cuda.synchronize()
+        for b in range(w.B):
+            Xo = oracle.step(X0[b], w.phase[b], 0.0, 0, 100, dataclasses.replace(p, system=b))
+            assert np.abs(out.cpu().numpy()[b].astype(np.float64) - Xo).max() <= tol * ELL
+        # the noise did move the spheres: far more than the tolerance
+        Xdet = oracle.step(X0[0], w.phase[0], 0.0, 0, 100, dataclasses.replace(p, kT=0.0))
+        assert np.abs(Xo * 0 + out.cpu().numpy()[0].astype(np.float64) - Xdet).max() > 1e-2
+
+
+def test_noise_at_headline_size_low_latency_path():
+    """N = 4096, FP32, 147 CTAs (tagged hand-over): 50 noisy Heun steps against the oracle."""
+    import dataclasses
+    w = inputs.config4()
+    Xg, X0, p = gpu_steps(w, ds.F32, 50, kT=0.01, seed=77)
+    Xo = oracle.step(X0[0], w.phase[0], 0.0, 0, 50, p)
+    assert np.abs(Xg[0] - Xo).max() <= 1e-4 * ELL
