@@ -70,6 +70,9 @@ def lib():
         L.or_philox4x32_10.argtypes = [ctypes.POINTER(ctypes.c_uint32)] * 3
         L.or_noise_normal.argtypes = [ctypes.c_uint64, ctypes.c_int64, ctypes.c_int32, ctypes.c_int64]
         L.or_noise_normal.restype = ctypes.c_double
+        L.or_avg_rhs.argtypes = [ctypes.c_int32, _dp, _dp, _dp, ctypes.POINTER(_CParams), _dp, _dp]
+        L.or_avg_step.argtypes = [ctypes.c_int32, _dp, _dp, _dp, ctypes.c_double, ctypes.c_int64, ctypes.POINTER(_CParams)]
+        L.or_avg_step.restype = ctypes.c_int
         L.or_dumbbell_coords.argtypes = [ctypes.c_int32, _dp, _dp, _dp]
         L.or_msd.argtypes = [ctypes.c_int32, ctypes.c_int32, _dp, _dp]
         L.or_msd.restype = ctypes.c_double
@@ -188,3 +191,27 @@ def philox4x32_10(ctr, key):
 def noise_normal(seed, n, system, element):
     """z ~ N(0,1) of step n, realisation `system`, state element 3 alpha + i (Eq. 1b, 1c)."""
     return float(lib().or_noise_normal(int(seed), int(n), int(system), int(element)))
+
+
+def avg_rhs(R, N, phi, p: Params):
+    """Stroke-averaged far-field model, Eq. (9a)-(9d): (dR/dt, dN/dt), each [S][3]."""
+    R, rp = _d(R)
+    N, np_ = _d(N)
+    phi, pp = _d(phi)
+    cp = p.c()
+    dR = np.empty_like(R)
+    dN = np.empty_like(N)
+    lib().or_avg_rhs(R.shape[0], rp, np_, pp, ctypes.byref(cp), dR.ctypes.data_as(_dp), dN.ctypes.data_as(_dp))
+    return dR, dN
+
+
+def avg_step(R, N, phi, dt, n_steps, p: Params):
+    """n_steps Heun steps of Eq. (9) with step dt (N renormalised after every stage): (R, N)."""
+    R = np.array(R, dtype=np.float64, order="C", copy=True)
+    N = np.array(N, dtype=np.float64, order="C", copy=True)
+    phi, pp = _d(phi)
+    cp = p.c()
+    rc = lib().or_avg_step(R.shape[0], R.ctypes.data_as(_dp), N.ctypes.data_as(_dp), pp, float(dt), int(n_steps), ctypes.byref(cp))
+    if rc:
+        raise MemoryError("or_avg_step")
+    return R, N

@@ -19,6 +19,7 @@
  *   or_velocity          forces followed by the mobility apply
  *   or_step              explicit Euler / one-step Heun predictor-corrector
  *   or_noise_normal      Eq. (1a-c), additive approximation of PAPER.md:240: the Gaussian increments (Philox4x32-10)
+ *   or_avg_rhs, or_avg_step   Eq. (9a-d) PAPER.md:121-135  the stroke-averaged far-field model and its Heun stepping
  *   or_dumbbell_coords   Eq. (6a,b) PAPER.md:87-91  direction and geometric centre of every dumbbell
  *   or_msd               Eq. (13)  PAPER.md:189     mean square displacement per particle over W realisations
  *
@@ -294,4 +295,74 @@ double or_msd(int32_t W, int32_t S, const double *Rt, const double *R0) {
         outer += inner / (double)S;
     }
     return outer / (double)W;
+}
+
+/* Stroke-averaged far-field model, Eq. (9a)-(9d), as printed (the numerical comparison with the
+ * microscopic model, pin P20, confirms the prefactors 9/64, 15/64 and the sign of (9b)):
+ *   dR^s/dt = sum_{r != s} J^{sr},      dN^s/dt = -(1 - N^s N^s) sum_{r != s} K^{sr},
+ *   J^{sr} = a w sin(phi^s - phi^r) (9/64) (lam/ell)^2 (ell/|D|)^4 { N^s (2s + 4qr - 10 s r^2)
+ *                                  + Dh (1 + 2q^2 - 5s^2 - 5r^2 - 20qsr + 35 s^2 r^2) },
+ *   K^{sr} = w sin(phi^s - phi^r) (15/64) (a/ell) (lam/ell)^2 (ell/|D|)^5 Dh (3s + 6rq + 6sq^2 - 7s^3 - 21 s r^2
+ *                                  - 42 q s^2 r + 63 s^3 r^2),
+ *   D = R^s - R^r, Dh = D/|D|, s = Dh.N^s, r = Dh.N^r, q = N^s.N^r   (9d; its printed indices are slips).
+ * R, N [S][3] -> dR, dN [S][3].  Plain double loops in the order of the formulas.                                  */
+void or_avg_rhs(int32_t S, const double *R, const double *N, const double *phi, const or_params *p, double *dR,
+                double *dN) {
+    const double a = p->a, ell = p->ell, lam = p->lambda, w = p->omega;
+    for (int32_t s_ = 0; s_ < S; ++s_) {
+        double Jsum[3] = {0, 0, 0}, Ksum[3] = {0, 0, 0};
+        const double *Ns = N + 3 * (size_t)s_;
+        for (int32_t r_ = 0; r_ < S; ++r_) {
+            if (r_ == s_) continue;
+            const double *Nr = N + 3 * (size_t)r_;
+            double D[3], Dn2 = 0.0;
+            for (int c = 0; c < 3; ++c) { D[c] = R[3 * (size_t)s_ + c] - R[3 * (size_t)r_ + c]; Dn2 += D[c] * D[c]; }
+            const double Dn = sqrt(Dn2);
+            double Dh[3], s = 0.0, r = 0.0, q = 0.0;
+            for (int c = 0; c < 3; ++c) { Dh[c] = D[c] / Dn; s += Dh[c] * Ns[c]; r += Dh[c] * Nr[c]; q += Ns[c] * Nr[c]; }
+            const double sn = sin(phi[s_] - phi[r_]);
+            const double lr = ell / Dn, ll = lam / ell;
+            const double cj = a * w * sn * (9.0 / 64.0) * ll * ll * lr * lr * lr * lr;
+            const double ck = w * sn * (15.0 / 64.0) * (a / ell) * ll * ll * lr * lr * lr * lr * lr;
+            const double jn = 2.0 * s + 4.0 * q * r - 10.0 * s * r * r;
+            const double jd = 1.0 + 2.0 * q * q - 5.0 * s * s - 5.0 * r * r - 20.0 * q * s * r + 35.0 * s * s * r * r;
+            const double kd = 3.0 * s + 6.0 * r * q + 6.0 * s * q * q - 7.0 * s * s * s - 21.0 * s * r * r - 42.0 * q * s * s * r +
+                              63.0 * s * s * s * r * r;
+            for (int c = 0; c < 3; ++c) {
+                Jsum[c] += cj * (Ns[c] * jn + Dh[c] * jd);
+                Ksum[c] += ck * Dh[c] * kd;
+            }
+        }
+        const double nk = Ns[0] * Ksum[0] + Ns[1] * Ksum[1] + Ns[2] * Ksum[2];
+        for (int c = 0; c < 3; ++c) {
+            dR[3 * (size_t)s_ + c] = Jsum[c];
+            dN[3 * (size_t)s_ + c] = -(Ksum[c] - Ns[c] * nk);
+        }
+    }
+}
+
+/* n_steps Heun steps of Eq. (9) with step dt (reading R16: the paper does not say how it integrates (9); the
+ * predictor-corrector of PAPER.md:236 is used, and N is renormalised after every stage because the projector of (9b)
+ * keeps |N| = 1 only to first order in dt).                                                                          */
+int or_avg_step(int32_t S, double *R, double *N, const double *phi, double dt, int64_t n_steps, const or_params *p) {
+    const size_t M = 3 * (size_t)S;
+    double *buf = (double *)malloc(6 * M * sizeof(double));
+    if (!buf) return -1;
+    double *dR1 = buf, *dN1 = buf + M, *dR2 = buf + 2 * M, *dN2 = buf + 3 * M, *Rp = buf + 4 * M, *Np = buf + 5 * M;
+    for (int64_t n = 0; n < n_steps; ++n) {
+        or_avg_rhs(S, R, N, phi, p, dR1, dN1);
+        for (size_t k = 0; k < M; ++k) { Rp[k] = R[k] + dt * dR1[k]; Np[k] = N[k] + dt * dN1[k]; }
+        for (int32_t s = 0; s < S; ++s) {
+            double *v = Np + 3 * (size_t)s; const double len = sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+            v[0] /= len; v[1] /= len; v[2] /= len;
+        }
+        or_avg_rhs(S, Rp, Np, phi, p, dR2, dN2);
+        for (size_t k = 0; k < M; ++k) { R[k] = R[k] + 0.5 * dt * (dR1[k] + dR2[k]); N[k] = N[k] + 0.5 * dt * (dN1[k] + dN2[k]); }
+        for (int32_t s = 0; s < S; ++s) {
+            double *v = N + 3 * (size_t)s; const double len = sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+            v[0] /= len; v[1] /= len; v[2] /= len;
+        }
+    }
+    free(buf);
+    return 0;
 }
