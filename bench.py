@@ -332,6 +332,30 @@ def extras(torch, ds, inputs, w, args, precision, tensor):
         cfgs[name] = {"timesteps_per_s": nst / t, "pairs_per_s": nst * 2 * pairs_per_apply(wc.N, wc.B) / t,
                       "steps_timed": nst}
     extra["configs_rpy_heun"] = cfgs
+    # the stroke-averaged far-field model (Eq. 9), the paper's comparison system: one right-hand side (S^2 dumbbell pairs)
+    avg = {}
+    for S_ in (729, 2048):
+        rng = np.random.default_rng(S_)
+        Rr = torch.as_tensor(rng.uniform(-200, 200, (S_, 3)).astype(np.float32), device="cuda")
+        Nr = rng.standard_normal((S_, 3)); Nr /= np.linalg.norm(Nr, axis=1, keepdims=True)
+        Nr = torch.as_tensor(Nr.astype(np.float32), device="cuda")
+        ph = torch.as_tensor(rng.uniform(0, 6.28, S_), device="cuda")
+        dRr, dNr = torch.empty_like(Rr), torch.empty_like(Nr)
+        with ds.System(1, precision=ds.F32, device=torch.cuda.current_device(),
+                       stream=torch.cuda.current_stream().cuda_stream) as sa:
+            for _ in range(3):
+                sa.avg_rhs(Rr, Nr, ph, dRr, dNr, S_)
+            torch.cuda.synchronize()
+            e0, e1 = _events(torch)
+            e0.record()
+            for _ in range(50):
+                sa.avg_rhs(Rr, Nr, ph, dRr, dNr, S_)
+            e1.record()
+            torch.cuda.synchronize()
+            t = e0.elapsed_time(e1) * 1e-3 / 50
+        avg[f"S{S_}"] = {"us_per_rhs": t * 1e6, "dumbbell_pairs_per_s": S_ * (S_ - 1) / t,
+                         "note": "ds_avg_rhs incl. its widen/narrow kernels, FP32 pair arithmetic, not tuned"}
+    extra["avg_model_eq9"] = avg
     extra["cold_l2"] = {"ms_per_step": 1e3 * time_steps_cold_l2(torch, ds, w, precision, tensor, 30),
                         "steps": 30, "flush": "512 MiB fill before every step"}
     if args.sweep:

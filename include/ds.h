@@ -141,6 +141,16 @@ int ds_dumbbell_coords(ds_system *s, void *R, void *Nv);
 int ds_msd_set_reference(ds_system *s);
 int ds_msd(ds_system *s, double *msd);
 
+/* Stroke-averaged far-field model, Eq. (9a)-(9d): the paper's comparison model, a second O(S^2) pair sum
+ * over dumbbells (centres R, unit directions Nv, stroke phases).  Stateless: S is any dumbbell count >= 1; a, ell, lambda,
+ * omega and the precision of the pair arithmetic come from the system; R, Nv, dR, dN are [S][3] in user precision, phase
+ * [S] double; device or host pointers.
+ *   ds_avg_rhs : dR = sum_r J^{sr},  dN = -(1 - N N) sum_r K^{sr}   (right-hand sides of (9a), (9b)).
+ *   ds_avg_step: n_steps Heun steps of size dt on R, Nv in place; the state is FP64 inside the call (the
+ *                increments are below FP32 resolution) and Nv is renormalised after every stage.      */
+int ds_avg_rhs(ds_system *s, const void *R, const void *Nv, const void *phase, void *dR, void *dN, int32_t S);
+int ds_avg_step(ds_system *s, void *R, void *Nv, const void *phase, int32_t S, double dt, int64_t n_steps);
+
 /* Launch-shape override for tuning and tests: number of row tiles (CTAs) per system; 0 = library
  * heuristic.  Values below ceil(ceil(N/4)/512) or above ceil(N/4) are clamped; the step modes also
  * clamp to the SM count (their CTAs meet at a barrier every stage and must be co-resident).      */

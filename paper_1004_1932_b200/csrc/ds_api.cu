@@ -14,6 +14,7 @@
 #include "../../include/ds.h"
 #include "mobility.cuh"
 #include "peak.cuh"
+#include "averaged.cuh"
 #include "state.cuh"
 
 namespace {
@@ -80,6 +81,7 @@ struct ds_system {
     long long *probe = nullptr;                 // caller's device buffer (ds_set_probe) or NULL
     // scratch of the stateless apply and of host-pointer staging
     Buf ap_units, st_a, st_b, st_c;
+    Buf avg;                                    // FP64 scratch of the stroke-averaged model (Eq. 9)
 };
 
 namespace {
@@ -361,6 +363,56 @@ template <typename T> int peak_probe_t(int num_sms, double *flops_per_s) {
 
 bool finite_pos(double x) { return isfinite(x) && x > 0.0; }
 
+ds::AvgConsts avg_consts(const ds_system *s) {
+    const double a = s->P.a, ell = s->P.ell, lam = s->P.lambda, w = s->P.omega, ll = lam / ell;
+    ds::AvgConsts C;
+    C.cj = a * w * (9.0 / 64.0) * ll * ll * ell * ell * ell * ell;
+    C.ck = w * (15.0 / 64.0) * (a / ell) * ll * ll * ell * ell * ell * ell * ell;
+    return C;
+}
+
+int launch_avg_rhs(ds_system *s, const double *R, const double *N, const double *phi, int S, double *dR, double *dN) {
+    const dim3 block(ds::AVG_SB, ds::AVG_SL), grid((unsigned)((S + ds::AVG_SB - 1) / ds::AVG_SB));
+    if (s->P.precision == DS_F64)
+        ds::avg_rhs_kernel<double><<<grid, block, 0, s->stream>>>(R, N, phi, S, avg_consts(s), dR, dN);
+    else
+        ds::avg_rhs_kernel<float><<<grid, block, 0, s->stream>>>(R, N, phi, S, avg_consts(s), dR, dN);
+    CU_TRY(cudaGetLastError());
+    s->launches += 1;
+    return DS_OK;
+}
+
+// user buffer (device or host, user precision, n elements) -> FP64 device array dst
+int avg_in(ds_system *s, const void *src, double *dst, size_t n, Buf &stage) {
+    const size_t nb = n * elem_size(s);
+    int dev = 0;
+    DS_TRY(is_device_ptr(src, &dev));
+    const void *d = src;
+    if (!dev) { DS_TRY(ensure(stage, nb)); CU_TRY(cudaMemcpyAsync(stage.p, src, nb, cudaMemcpyHostToDevice, s->stream)); d = stage.p; }
+    const unsigned g = (unsigned)((n + 255) / 256);
+    if (s->P.precision == DS_F64) ds::widen_kernel<double><<<g, 256, 0, s->stream>>>((const double *)d, dst, (long long)n);
+    else ds::widen_kernel<float><<<g, 256, 0, s->stream>>>((const float *)d, dst, (long long)n);
+    CU_TRY(cudaGetLastError());
+    s->launches += 1;
+    return DS_OK;
+}
+
+// FP64 device array -> user buffer; returns whether the caller must synchronise (host destination)
+int avg_out(ds_system *s, const double *src, void *dst, size_t n, Buf &stage, bool *host) {
+    const size_t nb = n * elem_size(s);
+    int dev = 0;
+    DS_TRY(is_device_ptr(dst, &dev));
+    void *d = dst;
+    if (!dev) { DS_TRY(ensure(stage, nb)); d = stage.p; }
+    const unsigned g = (unsigned)((n + 255) / 256);
+    if (s->P.precision == DS_F64) ds::narrow_kernel<double><<<g, 256, 0, s->stream>>>(src, (double *)d, (long long)n);
+    else ds::narrow_kernel<float><<<g, 256, 0, s->stream>>>(src, (float *)d, (long long)n);
+    CU_TRY(cudaGetLastError());
+    s->launches += 1;
+    if (!dev) { CU_TRY(cudaMemcpyAsync(dst, d, nb, cudaMemcpyDeviceToHost, s->stream)); *host = true; }
+    return DS_OK;
+}
+
 // X (FP64) <- xu (user precision) when only the latter is current (ds_set_state with a host buffer)
 int materialize_x(ds_system *s) {
     if (s->x_valid) return DS_OK;
@@ -458,7 +510,7 @@ int ds_destroy(ds_system *s) {
     cudaSetDevice(s->P.device);
     cudaStreamSynchronize(s->stream);
     void *ptrs[] = {s->X, s->xu, s->Rref, s->msd_part, s->msd_out, s->phase, s->units[0], s->units[1], s->ll[0], s->ll[1], s->bar, s->Xcg, s->V1g, s->Fg, s->Lg,
-                    s->ap_units.p, s->st_a.p, s->st_b.p, s->st_c.p};
+                    s->ap_units.p, s->st_a.p, s->st_b.p, s->st_c.p, s->avg.p};
     for (void *q : ptrs) if (q) cudaFree(q);
     (void)cudaGetLastError();
     delete s;
@@ -616,6 +668,55 @@ int ds_msd(ds_system *s, double *msd) {
         CU_TRY(cudaMemcpyAsync(msd, s->msd_out, sizeof(double), cudaMemcpyDeviceToHost, s->stream));
         CU_TRY(cudaStreamSynchronize(s->stream));
     }
+    return DS_OK;
+}
+
+int ds_avg_rhs(ds_system *s, const void *R, const void *Nv, const void *phase, void *dR, void *dN, int32_t S) {
+    if (!s || !R || !Nv || !phase || !dR || !dN) return DS_ERR_NULL;
+    if (S < 1) return DS_ERR_INVALID_PARAM;
+    DS_TRY(set_device(s));
+    const size_t M = 3 * (size_t)S;
+    DS_TRY(ensure(s->avg, (4 * M + (size_t)S) * sizeof(double)));
+    double *Rd = (double *)s->avg.p, *Nd = Rd + M, *dRd = Nd + M, *dNd = dRd + M, *phd = dNd + M;
+    int pdev = 0;
+    DS_TRY(is_device_ptr(phase, &pdev));
+    CU_TRY(cudaMemcpyAsync(phd, phase, (size_t)S * sizeof(double), pdev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s->stream));
+    DS_TRY(avg_in(s, R, Rd, M, s->st_a));
+    DS_TRY(avg_in(s, Nv, Nd, M, s->st_b));
+    DS_TRY(launch_avg_rhs(s, Rd, Nd, phd, S, dRd, dNd));
+    bool host = false;
+    DS_TRY(avg_out(s, dRd, dR, M, s->st_a, &host));
+    DS_TRY(avg_out(s, dNd, dN, M, s->st_b, &host));
+    if (host) CU_TRY(cudaStreamSynchronize(s->stream));
+    return DS_OK;
+}
+
+int ds_avg_step(ds_system *s, void *R, void *Nv, const void *phase, int32_t S, double dt, int64_t n_steps) {
+    if (!s || !R || !Nv || !phase) return DS_ERR_NULL;
+    if (S < 1 || n_steps < 0 || !isfinite(dt) || dt <= 0.0) return DS_ERR_INVALID_PARAM;
+    DS_TRY(set_device(s));
+    const size_t M = 3 * (size_t)S;
+    DS_TRY(ensure(s->avg, (8 * M + (size_t)S) * sizeof(double)));
+    double *Rd = (double *)s->avg.p, *Nd = Rd + M, *Rp = Nd + M, *Np = Rp + M, *dR1 = Np + M, *dN1 = dR1 + M, *dR2 = dN1 + M,
+           *dN2 = dR2 + M, *phd = dN2 + M;
+    int pdev = 0;
+    DS_TRY(is_device_ptr(phase, &pdev));
+    CU_TRY(cudaMemcpyAsync(phd, phase, (size_t)S * sizeof(double), pdev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s->stream));
+    DS_TRY(avg_in(s, R, Rd, M, s->st_a));
+    DS_TRY(avg_in(s, Nv, Nd, M, s->st_b));
+    const unsigned ug = (unsigned)((S + 127) / 128);
+    for (int64_t n = 0; n < n_steps; ++n) {
+        DS_TRY(launch_avg_rhs(s, Rd, Nd, phd, S, dR1, dN1));
+        ds::avg_update_kernel<<<ug, 128, 0, s->stream>>>(Rd, Nd, dR1, dN1, dR1, dN1, dt, 0, S, Rp, Np);
+        DS_TRY(launch_avg_rhs(s, Rp, Np, phd, S, dR2, dN2));
+        ds::avg_update_kernel<<<ug, 128, 0, s->stream>>>(Rd, Nd, dR1, dN1, dR2, dN2, dt, 1, S, Rd, Nd);
+        CU_TRY(cudaGetLastError());
+        s->launches += 2;
+    }
+    bool host = false;
+    DS_TRY(avg_out(s, Rd, R, M, s->st_a, &host));
+    DS_TRY(avg_out(s, Nd, Nv, M, s->st_b, &host));
+    if (host) CU_TRY(cudaStreamSynchronize(s->stream));
     return DS_OK;
 }
 

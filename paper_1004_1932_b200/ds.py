@@ -22,7 +22,7 @@ ERR_INVALID_PARAM, ERR_NULL, ERR_CUDA, ERR_STATE, ERR_NO_DEVICE, ERR_ALLOC = -1,
 
 # every symbol include/ds.h declares (tests check that the built library exports all of them)
 SYMBOLS = ["ds_create", "ds_destroy", "ds_set_stream", "ds_set_state", "ds_get_state", "ds_forces",
-           "ds_mobility_apply", "ds_step", "ds_batch_step", "ds_velocity", "ds_dumbbell_coords", "ds_msd_set_reference", "ds_msd", "ds_set_tuning", "ds_set_probe", "ds_launch_count",
+           "ds_mobility_apply", "ds_step", "ds_batch_step", "ds_velocity", "ds_dumbbell_coords", "ds_msd_set_reference", "ds_msd", "ds_avg_rhs", "ds_avg_step", "ds_set_tuning", "ds_set_probe", "ds_launch_count",
            "ds_peak_probe", "ds_strerror", "ds_last_cuda_error", "ds_version"]
 
 
@@ -65,6 +65,8 @@ def lib():
         L.ds_batch_step.argtypes = [vp, i64]
         L.ds_velocity.argtypes = [vp, vp]
         L.ds_dumbbell_coords.argtypes = [vp, vp, vp]
+        L.ds_avg_rhs.argtypes = [vp, vp, vp, vp, vp, vp, i32]
+        L.ds_avg_step.argtypes = [vp, vp, vp, vp, i32, dbl, i64]
         L.ds_msd_set_reference.argtypes = [vp]
         L.ds_msd.argtypes = [vp, ctypes.POINTER(dbl)]
         L.ds_set_tuning.argtypes = [vp, i32]
@@ -169,6 +171,12 @@ class System:
         v = ctypes.c_double()
         _check(lib().ds_msd(self._h, ctypes.byref(v)), "ds_msd")
         return v.value
+
+    def avg_rhs(self, R, Nv, phase, dR, dN, S):
+        _check(lib().ds_avg_rhs(self._h, _ptr(R), _ptr(Nv), _ptr(phase), _ptr(dR), _ptr(dN), int(S)), "ds_avg_rhs")
+
+    def avg_step(self, R, Nv, phase, S, dt, n_steps):
+        _check(lib().ds_avg_step(self._h, _ptr(R), _ptr(Nv), _ptr(phase), int(S), float(dt), int(n_steps)), "ds_avg_step")
 
     def mobility_apply(self, pos, F, u, n):
         _check(lib().ds_mobility_apply(self._h, _ptr(pos), _ptr(F), _ptr(u), int(n)), "ds_mobility_apply")

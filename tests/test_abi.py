@@ -54,7 +54,8 @@ def test_null_and_invalid_arguments_are_rejected_before_any_device_work():
                      (L.ds_forces, (None, None)), (L.ds_mobility_apply, (None, None, None, None, 4)),
                      (L.ds_step, (None, 1)), (L.ds_batch_step, (None, 1)), (L.ds_velocity, (None, None)),
                      (L.ds_set_tuning, (None, 0)), (L.ds_set_stream, (None, None)),
-                     (L.ds_dumbbell_coords, (None, None, None)), (L.ds_msd_set_reference, (None,)), (L.ds_msd, (None, None))]:
+                     (L.ds_dumbbell_coords, (None, None, None)), (L.ds_msd_set_reference, (None,)), (L.ds_msd, (None, None)),
+                     (L.ds_avg_rhs, (None, None, None, None, None, None, 4)), (L.ds_avg_step, (None, None, None, None, 4, 0.5, 1))]:
         assert fn(*args) == ds.ERR_NULL
     assert L.ds_destroy(None) == ds.OK
     assert L.ds_launch_count(None) == 0

@@ -537,3 +537,57 @@ def test_noise_at_headline_size_low_latency_path():
     Xg, X0, p = gpu_steps(w, ds.F32, 50, kT=0.01, seed=77)
     Xo = oracle.step(X0[0], w.phase[0], 0.0, 0, 50, p)
     assert np.abs(Xg[0] - Xo).max() <= 1e-4 * ELL
+
+
+# --------------------------------------------------------------------------------- stroke-averaged model, Eq. (9)
+def _avg_case(S, seed, side):
+    rng = np.random.default_rng(seed)
+    R = rng.uniform(-side / 2, side / 2, (S, 3))
+    N = rng.standard_normal((S, 3)); N /= np.linalg.norm(N, axis=1, keepdims=True)
+    return R, N, rng.uniform(0, 2 * np.pi, S)
+
+
+@pytest.mark.parametrize("precision", [ds.F32, ds.F64])
+@pytest.mark.parametrize("S", [1, 2, 33, 300, 729])
+def test_avg_rhs_parity(S, precision):
+    """Eq. (9a)-(9d) on the device against the oracle: S below one block, ragged, several tiles, and the paper's largest
+    lattice 9^3 = 729; device and host buffers."""
+    R, N, phi = _avg_case(S, 900 + S, 60.0 * max(S, 2) ** (1 / 3))
+    Rr, Nr = R.astype(NPDT[precision]), N.astype(NPDT[precision])
+    p = oracle.Params(a=0.8, ell=9.0, lam=1.7, omega=5.5)
+    dRo, dNo = oracle.avg_rhs(Rr.astype(np.float64), Nr.astype(np.float64), phi, p)
+    with ds.System(1, precision=precision, a=p.a, ell=p.ell, lam=p.lam, omega=p.omega) as s:
+        dR = torch.empty((S, 3), dtype=TDT[precision], device="cuda")
+        dN = np.empty((S, 3), dtype=NPDT[precision])
+        s.avg_rhs(dev(Rr, precision), np.ascontiguousarray(Nr), torch.as_tensor(phi, device="cuda"), dR, dN, S)
+        torch.cuda.synchronize()
+    if S == 1:
+        assert np.all(dR.cpu().numpy() == 0) and np.all(dN == 0)
+        return
+    tol = 2e-5 if precision == ds.F32 else 1e-12
+    assert rel_l2(dR.cpu().numpy().astype(np.float64), dRo) <= tol
+    assert rel_l2(dN.astype(np.float64), dNo) <= tol
+
+
+@pytest.mark.parametrize("precision,tol", [(ds.F64, 1e-12), (ds.F32, 1e-5)])
+def test_avg_step_parity_lattice(precision, tol):
+    """5 x 5 x 5 lattice of the paper's Fig. 3, random directions and phases: 40 Heun steps of half a
+    period each of the averaged model on the device against the oracle; the FP64 state keeps the tiny increments even
+    when the pair arithmetic is FP32, and N stays on the unit sphere."""
+    g = np.arange(5) * 30.0
+    R = np.stack(np.meshgrid(g, g, g, indexing="ij"), -1).reshape(-1, 3)
+    _, N, phi = _avg_case(125, 5, 1.0)
+    p = oracle.Params()
+    Ro, No = oracle.avg_step(R, N, phi, 0.5, 40, p)
+    with ds.System(1, precision=precision) as s:
+        Rd = dev(R, precision); Nd = dev(N, precision)
+        s.avg_step(Rd, Nd, torch.as_tensor(phi, device="cuda"), 125, 0.5, 40)
+        torch.cuda.synchronize()
+    Rg, Ng = Rd.cpu().numpy().astype(np.float64), Nd.cpu().numpy().astype(np.float64)
+    disp = np.abs(Ro - R).max()
+    if precision == ds.F64:
+        assert np.abs(Rg - Ro).max() <= tol * 120 and np.abs(Ng - No).max() <= tol
+        assert np.abs(Rg - R).max() > 0.5 * disp > 0
+    else:   # the output buffers are float32: the comparison is limited by their rounding, not by the stepping
+        assert np.abs(Rg - Ro).max() <= 120 * 6e-8 * 2 and np.abs(Ng - No).max() <= tol
+    np.testing.assert_allclose(np.linalg.norm(Ng, axis=1), 1.0, rtol=0, atol=3e-7 if precision == ds.F32 else 1e-15)
