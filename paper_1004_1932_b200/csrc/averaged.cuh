@@ -21,10 +21,12 @@ struct AvgConsts {
 
 constexpr int AVG_SB = 32, AVG_SL = 8, AVG_TILE = 256;
 
-template <typename T>
-__global__ void __launch_bounds__(AVG_SB *AVG_SL) avg_rhs_kernel(const double *__restrict__ R, const double *__restrict__ N,
+// T: type of the pair arithmetic; IO: element type of R, N, dR, dN (double for the FP64 state of ds_avg_step, the user's
+// type for the stateless ds_avg_rhs)
+template <typename T, typename IO>
+__global__ void __launch_bounds__(AVG_SB *AVG_SL) avg_rhs_kernel(const IO *__restrict__ R, const IO *__restrict__ N,
                                                                   const double *__restrict__ phi, int S, AvgConsts C,
-                                                                  double *__restrict__ dR, double *__restrict__ dN) {
+                                                                  IO *__restrict__ dR, IO *__restrict__ dN) {
     __shared__ T tR[AVG_TILE][3], tN[AVG_TILE][3], tS[AVG_TILE], tC[AVG_TILE];
     __shared__ T part[AVG_SL][AVG_SB][6];
     const int ls = threadIdx.x, sl = threadIdx.y, tid = sl * AVG_SB + ls;
@@ -80,10 +82,11 @@ __global__ void __launch_bounds__(AVG_SB *AVG_SL) avg_rhs_kernel(const double *_
             for (int m = 0; m < AVG_SL; ++m) { a += (double)part[m][ls][c]; b += (double)part[m][ls][3 + c]; }
             Js[c] = a; Ks[c] = b;
         }
-        const double n0 = N[3 * (size_t)s_], n1 = N[3 * (size_t)s_ + 1], n2 = N[3 * (size_t)s_ + 2];
+        const double n0 = (double)N[3 * (size_t)s_], n1 = (double)N[3 * (size_t)s_ + 1], n2 = (double)N[3 * (size_t)s_ + 2];
         const double nk = n0 * Ks[0] + n1 * Ks[1] + n2 * Ks[2];
-        dR[3 * (size_t)s_] = Js[0]; dR[3 * (size_t)s_ + 1] = Js[1]; dR[3 * (size_t)s_ + 2] = Js[2];
-        dN[3 * (size_t)s_] = -(Ks[0] - n0 * nk); dN[3 * (size_t)s_ + 1] = -(Ks[1] - n1 * nk); dN[3 * (size_t)s_ + 2] = -(Ks[2] - n2 * nk);
+        dR[3 * (size_t)s_] = (IO)Js[0]; dR[3 * (size_t)s_ + 1] = (IO)Js[1]; dR[3 * (size_t)s_ + 2] = (IO)Js[2];
+        dN[3 * (size_t)s_] = (IO)(-(Ks[0] - n0 * nk)); dN[3 * (size_t)s_ + 1] = (IO)(-(Ks[1] - n1 * nk));
+        dN[3 * (size_t)s_ + 2] = (IO)(-(Ks[2] - n2 * nk));
     }
 }
 

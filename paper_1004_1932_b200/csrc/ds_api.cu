@@ -371,12 +371,14 @@ ds::AvgConsts avg_consts(const ds_system *s) {
     return C;
 }
 
-int launch_avg_rhs(ds_system *s, const double *R, const double *N, const double *phi, int S, double *dR, double *dN) {
+// IO = double: the FP64 state of ds_avg_step; IO = the user's type: the stateless ds_avg_rhs on device buffers
+template <typename IO>
+int launch_avg_rhs(ds_system *s, const IO *R, const IO *N, const double *phi, int S, IO *dR, IO *dN) {
     const dim3 block(ds::AVG_SB, ds::AVG_SL), grid((unsigned)((S + ds::AVG_SB - 1) / ds::AVG_SB));
     if (s->P.precision == DS_F64)
-        ds::avg_rhs_kernel<double><<<grid, block, 0, s->stream>>>(R, N, phi, S, avg_consts(s), dR, dN);
+        ds::avg_rhs_kernel<double, IO><<<grid, block, 0, s->stream>>>(R, N, phi, S, avg_consts(s), dR, dN);
     else
-        ds::avg_rhs_kernel<float><<<grid, block, 0, s->stream>>>(R, N, phi, S, avg_consts(s), dR, dN);
+        ds::avg_rhs_kernel<float, IO><<<grid, block, 0, s->stream>>>(R, N, phi, S, avg_consts(s), dR, dN);
     CU_TRY(cudaGetLastError());
     s->launches += 1;
     return DS_OK;
@@ -675,19 +677,34 @@ int ds_avg_rhs(ds_system *s, const void *R, const void *Nv, const void *phase, v
     if (!s || !R || !Nv || !phase || !dR || !dN) return DS_ERR_NULL;
     if (S < 1) return DS_ERR_INVALID_PARAM;
     DS_TRY(set_device(s));
-    const size_t M = 3 * (size_t)S;
-    DS_TRY(ensure(s->avg, (4 * M + (size_t)S) * sizeof(double)));
-    double *Rd = (double *)s->avg.p, *Nd = Rd + M, *dRd = Nd + M, *dNd = dRd + M, *phd = dNd + M;
-    int pdev = 0;
-    DS_TRY(is_device_ptr(phase, &pdev));
-    CU_TRY(cudaMemcpyAsync(phd, phase, (size_t)S * sizeof(double), pdev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s->stream));
-    DS_TRY(avg_in(s, R, Rd, M, s->st_a));
-    DS_TRY(avg_in(s, Nv, Nd, M, s->st_b));
-    DS_TRY(launch_avg_rhs(s, Rd, Nd, phd, S, dRd, dNd));
-    bool host = false;
-    DS_TRY(avg_out(s, dRd, dR, M, s->st_a, &host));
-    DS_TRY(avg_out(s, dNd, dN, M, s->st_b, &host));
-    if (host) CU_TRY(cudaStreamSynchronize(s->stream));
+    const size_t M = 3 * (size_t)S, nb = M * elem_size(s);
+    // host buffers are staged through device scratch in the user's precision; device buffers are used in place
+    int dv[5];
+    const void *in[3] = {R, Nv, phase};
+    void *outp[2] = {dR, dN};
+    for (int k = 0; k < 3; ++k) DS_TRY(is_device_ptr(in[k], &dv[k]));
+    for (int k = 0; k < 2; ++k) DS_TRY(is_device_ptr(outp[k], &dv[3 + k]));
+    DS_TRY(ensure(s->avg, 4 * nb + (size_t)S * sizeof(double) + 64));
+    char *scr = (char *)s->avg.p;
+    const void *dRin = R, *dNin = Nv;
+    const double *dph = (const double *)phase;
+    void *dRo = dR, *dNo = dN;
+    if (!dv[0]) { CU_TRY(cudaMemcpyAsync(scr, R, nb, cudaMemcpyHostToDevice, s->stream)); dRin = scr; }
+    if (!dv[1]) { CU_TRY(cudaMemcpyAsync(scr + nb, Nv, nb, cudaMemcpyHostToDevice, s->stream)); dNin = scr + nb; }
+    if (!dv[2]) {
+        double *p = (double *)(scr + 4 * nb + ((8 - (4 * nb) % 8) % 8));
+        CU_TRY(cudaMemcpyAsync(p, phase, (size_t)S * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+        dph = p;
+    }
+    if (!dv[3]) dRo = scr + 2 * nb;
+    if (!dv[4]) dNo = scr + 3 * nb;
+    if (s->P.precision == DS_F64)
+        DS_TRY(launch_avg_rhs<double>(s, (const double *)dRin, (const double *)dNin, dph, S, (double *)dRo, (double *)dNo));
+    else
+        DS_TRY(launch_avg_rhs<float>(s, (const float *)dRin, (const float *)dNin, dph, S, (float *)dRo, (float *)dNo));
+    if (!dv[3]) CU_TRY(cudaMemcpyAsync(dR, dRo, nb, cudaMemcpyDeviceToHost, s->stream));
+    if (!dv[4]) CU_TRY(cudaMemcpyAsync(dN, dNo, nb, cudaMemcpyDeviceToHost, s->stream));
+    if (!dv[3] || !dv[4]) CU_TRY(cudaStreamSynchronize(s->stream));
     return DS_OK;
 }
 
@@ -706,9 +723,9 @@ int ds_avg_step(ds_system *s, void *R, void *Nv, const void *phase, int32_t S, d
     DS_TRY(avg_in(s, Nv, Nd, M, s->st_b));
     const unsigned ug = (unsigned)((S + 127) / 128);
     for (int64_t n = 0; n < n_steps; ++n) {
-        DS_TRY(launch_avg_rhs(s, Rd, Nd, phd, S, dR1, dN1));
+        DS_TRY(launch_avg_rhs<double>(s, Rd, Nd, phd, S, dR1, dN1));
         ds::avg_update_kernel<<<ug, 128, 0, s->stream>>>(Rd, Nd, dR1, dN1, dR1, dN1, dt, 0, S, Rp, Np);
-        DS_TRY(launch_avg_rhs(s, Rp, Np, phd, S, dR2, dN2));
+        DS_TRY(launch_avg_rhs<double>(s, Rp, Np, phd, S, dR2, dN2));
         ds::avg_update_kernel<<<ug, 128, 0, s->stream>>>(Rd, Nd, dR1, dN1, dR2, dN2, dt, 1, S, Rd, Nd);
         CU_TRY(cudaGetLastError());
         s->launches += 2;
