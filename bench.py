@@ -354,7 +354,7 @@ def extras(torch, ds, inputs, w, args, precision, tensor):
             torch.cuda.synchronize()
             t = e0.elapsed_time(e1) * 1e-3 / 50
         avg[f"S{S_}"] = {"us_per_rhs": t * 1e6, "dumbbell_pairs_per_s": S_ * (S_ - 1) / t,
-                         "note": "ds_avg_rhs on device buffers: one kernel, FP32 pair arithmetic, 32 dumbbells x 8 slices per CTA, not tuned"}
+                         "note": "ds_avg_rhs on device buffers: one kernel, FP32 pair arithmetic, 16 dumbbells x 16 slices per CTA, not tuned"}
     extra["avg_model_eq9"] = avg
     extra["cold_l2"] = {"ms_per_step": 1e3 * time_steps_cold_l2(torch, ds, w, precision, tensor, 30),
                         "steps": 30, "flush": "512 MiB fill before every step"}

@@ -7,7 +7,7 @@
 //                                  - 42 q s^2 r + 63 s^3 r^2),
 //   D = R^s - R^r, Dh = D/|D|, s = Dh.N^s, r = Dh.N^r, q = N^s.N^r.
 // The state (R, N) is FP64 (the increments per step are ~1e-7 of |R|: below FP32 resolution); the pair
-// arithmetic runs in T.  Block = 32 dumbbells s x 8 slices of the r loop; r tiles of 256 staged in shared memory with
+// arithmetic runs in T.  Block = 16 dumbbells s x 16 slices of the r loop; r tiles of 256 staged in shared memory with
 // sin/cos of the phases (sin(phi^s - phi^r) by the addition theorem: no transcendental per pair).
 #pragma once
 #include <cuda_runtime.h>
@@ -19,7 +19,10 @@ struct AvgConsts {
     double ck;   // w (15/64) (a/ell) (lam/ell)^2 ell^5
 };
 
-constexpr int AVG_SB = 32, AVG_SL = 8, AVG_TILE = 256;
+constexpr int AVG_SB = 16, AVG_SL = 16, AVG_TILE = 256;
+
+__device__ __forceinline__ float inv_sqrt(float x) { return rsqrtf(x); }
+__device__ __forceinline__ double inv_sqrt(double x) { return 1.0 / sqrt(x); }
 
 // T: type of the pair arithmetic; IO: element type of R, N, dR, dN (double for the FP64 state of ds_avg_step, the user's
 // type for the stateless ds_avg_rhs)
@@ -55,7 +58,7 @@ __global__ void __launch_bounds__(AVG_SB *AVG_SL) avg_rhs_kernel(const IO *__res
             if (t0 + k == s_ || !live) continue;
             const T D0 = Rs[0] - tR[k][0], D1 = Rs[1] - tR[k][1], D2 = Rs[2] - tR[k][2];
             const T d2 = D0 * D0 + D1 * D1 + D2 * D2;
-            const T di = (T)1 / sqrt(d2);
+            const T di = inv_sqrt(d2);
             const T h0 = D0 * di, h1 = D1 * di, h2 = D2 * di;
             const T s = h0 * Ns[0] + h1 * Ns[1] + h2 * Ns[2];
             const T r = h0 * tN[k][0] + h1 * tN[k][1] + h2 * tN[k][2];
