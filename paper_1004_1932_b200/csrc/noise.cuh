@@ -16,7 +16,7 @@ __device__ __forceinline__ void philox_round(uint32_t (&c)[4], uint32_t k0, uint
     c[0] = n0; c[1] = lo1; c[2] = n2; c[3] = lo0;
 }
 
-__device__ __forceinline__ double noise_normal(unsigned long long seed, long long n, int system, long long element) {
+__device__ __noinline__ double noise_normal(unsigned long long seed, long long n, int system, long long element) {
     uint32_t c[4] = {(uint32_t)((unsigned long long)n & 0xffffffffu), (uint32_t)((unsigned long long)n >> 32), (uint32_t)element,
                      (uint32_t)system};
     uint32_t k0 = (uint32_t)(seed & 0xffffffffu), k1 = (uint32_t)(seed >> 32);
