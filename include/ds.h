@@ -84,7 +84,7 @@ typedef struct {
     uint64_t seed;       /* key of the generator (the library itself keeps no random state)        */
 } ds_params;
 
-/* Validate p, allocate the system's device buffers and build its CUDA graphs.
+/* Validate p, allocate the system's device buffers and choose its launch shape.
  * Rejects (DS_ERR_INVALID_PARAM): S < 1, B < 1, unknown enum values, non-positive or non-finite
  * a, eta, k0, dt, ell, negative omega, negative or non-finite kT, and ell <= 2a + |lambda|.               */
 int ds_create(const ds_params *p, ds_system **out);

@@ -1,5 +1,5 @@
 // ds_api.cu -- host runtime behind the C ABI of include/ds.h: parameter validation, device
-// buffers, host/device pointer staging, launch-shape choice, CUDA-graph build and replay.
+// buffers, host/device pointer staging, launch-shape choice, kernel-variant dispatch.
 // No arithmetic of the method lives here; it is all in mobility.cuh / state.cuh.
 #include <cuda_runtime.h>
 #include <math.h>
