@@ -334,7 +334,7 @@ def extras(torch, ds, inputs, w, args, precision, tensor):
     extra["configs_rpy_heun"] = cfgs
     # the stroke-averaged far-field model (Eq. 9), the paper's comparison system: one right-hand side (S^2 dumbbell pairs)
     avg = {}
-    for S_ in (729, 2048):
+    for S_ in (729, 2048, 8192):
         rng = np.random.default_rng(S_)
         Rr = torch.as_tensor(rng.uniform(-200, 200, (S_, 3)).astype(np.float32), device="cuda")
         Nr = rng.standard_normal((S_, 3)); Nr /= np.linalg.norm(Nr, axis=1, keepdims=True)
@@ -353,8 +353,19 @@ def extras(torch, ds, inputs, w, args, precision, tensor):
             e1.record()
             torch.cuda.synchronize()
             t = e0.elapsed_time(e1) * 1e-3 / 50
+            nst = 400
+            sa.avg_step(Rr, Nr, ph, S_, 0.5, 8)
+            torch.cuda.synchronize()
+            e0.record()
+            sa.avg_step(Rr, Nr, ph, S_, 0.5, nst)
+            e1.record()
+            torch.cuda.synchronize()
+            ts = e0.elapsed_time(e1) * 1e-3 / nst
         avg[f"S{S_}"] = {"us_per_rhs": t * 1e6, "dumbbell_pairs_per_s": S_ * (S_ - 1) / t,
-                         "note": "ds_avg_rhs on device buffers: one kernel, FP32 pair arithmetic, 16 dumbbells x 16 slices per CTA, not tuned"}
+                         "us_per_heun_step": ts * 1e6, "dumbbell_pairs_per_s_stepping": 2 * S_ * (S_ - 1) / ts,
+                         "note": "ds_avg_rhs on device buffers (sin/cos table kernel + pair kernel per call) and ds_avg_step "
+                                 "(2 launches per Heun step, FP64 state); FP32 pair arithmetic, 32 dumbbells x 8 slices per "
+                                 "CTA, clusters of <= 8 CTAs per block of dumbbells"}
     extra["avg_model_eq9"] = avg
     extra["cold_l2"] = {"ms_per_step": 1e3 * time_steps_cold_l2(torch, ds, w, precision, tensor, 30),
                         "steps": 30, "flush": "512 MiB fill before every step"}

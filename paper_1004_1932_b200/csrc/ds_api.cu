@@ -82,6 +82,7 @@ struct ds_system {
     // scratch of the stateless apply and of host-pointer staging
     Buf ap_units, st_a, st_b, st_c;
     Buf avg;                                    // FP64 scratch of the stroke-averaged model (Eq. 9)
+    Buf avg_sc;                                 // its sin/cos table
 };
 
 namespace {
@@ -371,17 +372,45 @@ ds::AvgConsts avg_consts(const ds_system *s) {
     return C;
 }
 
-// IO = double: the FP64 state of ds_avg_step; IO = the user's type: the stateless ds_avg_rhs on device buffers
-template <typename IO>
-int launch_avg_rhs(ds_system *s, const IO *R, const IO *N, const double *phi, int S, IO *dR, IO *dN) {
-    const dim3 block(ds::AVG_SB, ds::AVG_SL), grid((unsigned)((S + ds::AVG_SB - 1) / ds::AVG_SB));
-    if (s->P.precision == DS_F64)
-        ds::avg_rhs_kernel<double, IO><<<grid, block, 0, s->stream>>>(R, N, phi, S, avg_consts(s), dR, dN);
-    else
-        ds::avg_rhs_kernel<float, IO><<<grid, block, 0, s->stream>>>(R, N, phi, S, avg_consts(s), dR, dN);
+// sin/cos of the phases (device pointer) into s->avg_sc
+int avg_sincos(ds_system *s, const double *dphi, int S) {
+    DS_TRY(ensure(s->avg_sc, (size_t)S * sizeof(double2)));
+    ds::avg_sincos_kernel<<<(unsigned)((S + 127) / 128), 128, 0, s->stream>>>(dphi, S, (double2 *)s->avg_sc.p);
     CU_TRY(cudaGetLastError());
     s->launches += 1;
     return DS_OK;
+}
+
+// One evaluation of the right-hand sides of Eq. (9a,b).  The r sum is split into Y <= 8 chunks, one CTA of a cluster
+// each (S / 32 blocks alone would leave most SMs idle at the paper's S = 729).
+template <typename T, typename IO>
+int launch_avg_rhs_t(ds_system *s, const IO *R, const IO *N, int S, IO *dR, IO *dN, const ds::AvgUpdate &U) {
+    auto kern = ds::avg_rhs_kernel<T, IO>;
+    const int X = (S + ds::AVG_SB - 1) / ds::AVG_SB, slots = 4 * s->num_sms;
+    int Y = std::max(1, std::min(std::min(slots / X, ds::AVG_YMAX), (S + ds::AVG_W - 1) / ds::AVG_W));
+    int chunk = (S + Y - 1) / Y;
+    chunk = (chunk + ds::AVG_W - 1) / ds::AVG_W * ds::AVG_W;
+    Y = (S + chunk - 1) / chunk;
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof cfg);
+    cfg.gridDim = dim3((unsigned)X, (unsigned)Y); cfg.blockDim = dim3(ds::AVG_NT); cfg.stream = s->stream;
+    cudaLaunchAttribute at[2];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    at[1].id = cudaLaunchAttributeClusterDimension;
+    at[1].val.clusterDim.x = 1; at[1].val.clusterDim.y = (unsigned)Y; at[1].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = Y > 1 ? 2 : 1;
+    CU_TRY(cudaLaunchKernelEx(&cfg, kern, R, N, (const double2 *)s->avg_sc.p, S, chunk, avg_consts(s), dR, dN, U));
+    s->launches += 1;
+    return DS_OK;
+}
+
+// IO = double: the FP64 state of ds_avg_step; IO = the user's type: the stateless ds_avg_rhs on device buffers.
+// avg_sincos() must have run on the phases first.
+template <typename IO>
+int launch_avg_rhs(ds_system *s, const IO *R, const IO *N, int S, IO *dR, IO *dN, const ds::AvgUpdate &U = ds::AvgUpdate{}) {
+    if (s->P.precision == DS_F64) return launch_avg_rhs_t<double, IO>(s, R, N, S, dR, dN, U);
+    return launch_avg_rhs_t<float, IO>(s, R, N, S, dR, dN, U);
 }
 
 // user buffer (device or host, user precision, n elements) -> FP64 device array dst
@@ -512,7 +541,7 @@ int ds_destroy(ds_system *s) {
     cudaSetDevice(s->P.device);
     cudaStreamSynchronize(s->stream);
     void *ptrs[] = {s->X, s->xu, s->Rref, s->msd_part, s->msd_out, s->phase, s->units[0], s->units[1], s->ll[0], s->ll[1], s->bar, s->Xcg, s->V1g, s->Fg, s->Lg,
-                    s->ap_units.p, s->st_a.p, s->st_b.p, s->st_c.p, s->avg.p};
+                    s->ap_units.p, s->st_a.p, s->st_b.p, s->st_c.p, s->avg.p, s->avg_sc.p};
     for (void *q : ptrs) if (q) cudaFree(q);
     (void)cudaGetLastError();
     delete s;
@@ -698,10 +727,11 @@ int ds_avg_rhs(ds_system *s, const void *R, const void *Nv, const void *phase, v
     }
     if (!dv[3]) dRo = scr + 2 * nb;
     if (!dv[4]) dNo = scr + 3 * nb;
+    DS_TRY(avg_sincos(s, dph, S));
     if (s->P.precision == DS_F64)
-        DS_TRY(launch_avg_rhs<double>(s, (const double *)dRin, (const double *)dNin, dph, S, (double *)dRo, (double *)dNo));
+        DS_TRY(launch_avg_rhs<double>(s, (const double *)dRin, (const double *)dNin, S, (double *)dRo, (double *)dNo));
     else
-        DS_TRY(launch_avg_rhs<float>(s, (const float *)dRin, (const float *)dNin, dph, S, (float *)dRo, (float *)dNo));
+        DS_TRY(launch_avg_rhs<float>(s, (const float *)dRin, (const float *)dNin, S, (float *)dRo, (float *)dNo));
     if (!dv[3]) CU_TRY(cudaMemcpyAsync(dR, dRo, nb, cudaMemcpyDeviceToHost, s->stream));
     if (!dv[4]) CU_TRY(cudaMemcpyAsync(dN, dNo, nb, cudaMemcpyDeviceToHost, s->stream));
     if (!dv[3] || !dv[4]) CU_TRY(cudaStreamSynchronize(s->stream));
@@ -713,22 +743,20 @@ int ds_avg_step(ds_system *s, void *R, void *Nv, const void *phase, int32_t S, d
     if (S < 1 || n_steps < 0 || !isfinite(dt) || dt <= 0.0) return DS_ERR_INVALID_PARAM;
     DS_TRY(set_device(s));
     const size_t M = 3 * (size_t)S;
-    DS_TRY(ensure(s->avg, (8 * M + (size_t)S) * sizeof(double)));
-    double *Rd = (double *)s->avg.p, *Nd = Rd + M, *Rp = Nd + M, *Np = Rp + M, *dR1 = Np + M, *dN1 = dR1 + M, *dR2 = dN1 + M,
-           *dN2 = dR2 + M, *phd = dN2 + M;
+    DS_TRY(ensure(s->avg, (6 * M + (size_t)S) * sizeof(double)));
+    double *Rd = (double *)s->avg.p, *Nd = Rd + M, *Rp = Nd + M, *Np = Rp + M, *dR1 = Np + M, *dN1 = dR1 + M, *phd = dN1 + M;
     int pdev = 0;
     DS_TRY(is_device_ptr(phase, &pdev));
     CU_TRY(cudaMemcpyAsync(phd, phase, (size_t)S * sizeof(double), pdev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s->stream));
+    DS_TRY(avg_sincos(s, phd, S));
     DS_TRY(avg_in(s, R, Rd, M, s->st_a));
     DS_TRY(avg_in(s, Nv, Nd, M, s->st_b));
-    const unsigned ug = (unsigned)((S + 127) / 128);
+    // Heun: two launches per step, the update of a block of dumbbells done by the CTA that completes
+    // its right-hand sides (averaged.cuh)
+    ds::AvgUpdate P1{ds::AVG_PRED, dt, Rd, Nd, dR1, dN1, Rp, Np}, P2{ds::AVG_CORR, dt, Rd, Nd, dR1, dN1, Rd, Nd};
     for (int64_t n = 0; n < n_steps; ++n) {
-        DS_TRY(launch_avg_rhs<double>(s, Rd, Nd, phd, S, dR1, dN1));
-        ds::avg_update_kernel<<<ug, 128, 0, s->stream>>>(Rd, Nd, dR1, dN1, dR1, dN1, dt, 0, S, Rp, Np);
-        DS_TRY(launch_avg_rhs<double>(s, Rp, Np, phd, S, dR2, dN2));
-        ds::avg_update_kernel<<<ug, 128, 0, s->stream>>>(Rd, Nd, dR1, dN1, dR2, dN2, dt, 1, S, Rd, Nd);
-        CU_TRY(cudaGetLastError());
-        s->launches += 2;
+        DS_TRY(launch_avg_rhs<double>(s, Rd, Nd, S, (double *)nullptr, (double *)nullptr, P1));
+        DS_TRY(launch_avg_rhs<double>(s, Rp, Np, S, (double *)nullptr, (double *)nullptr, P2));
     }
     bool host = false;
     DS_TRY(avg_out(s, Rd, R, M, s->st_a, &host));

@@ -548,10 +548,11 @@ def _avg_case(S, seed, side):
 
 
 @pytest.mark.parametrize("precision", [ds.F32, ds.F64])
-@pytest.mark.parametrize("S", [1, 2, 33, 300, 729])
+@pytest.mark.parametrize("S", [1, 2, 9, 33, 300, 729, 2500, 9600])
 def test_avg_rhs_parity(S, precision):
-    """Eq. (9a)-(9d) on the device against the oracle: S below one block, ragged, several tiles, and the paper's largest
-    lattice 9^3 = 729; device and host buffers."""
+    """Eq. (9a)-(9d) on the device against the oracle: S below one block, a cluster whose last CTA holds one dumbbell
+    (9), ragged chunks, the paper's largest lattice 9^3 = 729, chunks of more than one shared-memory
+    tile (2500) and the single-CTA-per-block grid of large S (9600); device and host buffers."""
     R, N, phi = _avg_case(S, 900 + S, 60.0 * max(S, 2) ** (1 / 3))
     Rr, Nr = R.astype(NPDT[precision]), N.astype(NPDT[precision])
     p = oracle.Params(a=0.8, ell=9.0, lam=1.7, omega=5.5)
@@ -591,3 +592,27 @@ def test_avg_step_parity_lattice(precision, tol):
     else:   # the output buffers are float32: the comparison is limited by their rounding, not by the stepping
         assert np.abs(Rg - Ro).max() <= 120 * 6e-8 * 2 and np.abs(Ng - No).max() <= tol
     np.testing.assert_allclose(np.linalg.norm(Ng, axis=1), 1.0, rtol=0, atol=3e-7 if precision == ds.F32 else 1e-15)
+
+
+@pytest.mark.parametrize("precision", [ds.F64, ds.F32])
+def test_avg_step_parity_729(precision):
+    """The paper's largest lattice, 9 x 9 x 9, sites displaced by up to 5 (no close pairs: Eq. (9) is a
+    far-field model), random directions and phases: 6 Heun steps from the state as rounded to the working precision;
+    every s block is a cluster of 8 CTAs and the CTA that adds their sums also applies the predictor / corrector."""
+    S = 729
+    g = np.arange(9) * 30.0
+    jit, N, phi = _avg_case(S, 31, 10.0)
+    R = (np.stack(np.meshgrid(g, g, g, indexing="ij"), -1).reshape(-1, 3) + jit).astype(NPDT[precision]).astype(np.float64)
+    N = N.astype(NPDT[precision]).astype(np.float64)
+    p = oracle.Params()
+    Ro, No = oracle.avg_step(R, N, phi, 0.5, 6, p)
+    with ds.System(1, precision=precision) as s:
+        Rd = torch.as_tensor(R, device="cuda").to(TDT[precision]); Nd = torch.as_tensor(N, device="cuda").to(TDT[precision])
+        s.avg_step(Rd, Nd, phi, S, 0.5, 6)
+        torch.cuda.synchronize()
+    Rg, Ng = Rd.cpu().numpy().astype(np.float64), Nd.cpu().numpy().astype(np.float64)
+    assert np.abs(Ro - R).max() > 0
+    if precision == ds.F64:
+        assert np.abs(Rg - Ro).max() <= 1e-12 * 250 and np.abs(Ng - No).max() <= 1e-12
+    else:   # float32 output buffers: half an ulp of 250 is 1.5e-5
+        assert np.abs(Rg - Ro).max() <= 2e-5 and np.abs(Ng - No).max() <= 1e-5
