@@ -303,38 +303,11 @@ def workload_config(w, args, dtype):
                   "(512 MiB flush before every step) is in extra.cold_l2"}
 
 
-def extras(torch, ds, inputs, w, args, precision, tensor):
-    """Beside the headline: the standalone apply at N = 4096 (4 variants), timesteps/s of every config,
-    the cold-L2 per-step figure, and (with --sweep) the N = 256 .. 65536 apply sweep."""
-    extra = {}
-    # apply at N = 4096, all four variants (the standalone sweep of config 4)
-    Xa, Fa = inputs.apply_case(4096, 1004, 2004)
-    ap = {}
-    for pname, pr in (("f32", ds.F32), ("f64", ds.F64)):
-        for tname, tn in (("oseen", ds.OSEEN), ("rpy", ds.RPY)):
-            t = time_apply(torch, ds, 4096, pr, tn, Xa, Fa, reps=200)
-            ln = F32_LANES if pname == "f32" else F64_LANES
-            ap[f"{pname}_{tname}"] = {"us": t * 1e6, "pairs_per_s": pairs_per_apply(4096) / t,
-                                      "frac_of_alu_peak": pairs_per_apply(4096) * FLOP_PER_PAIR[tname] / t /
-                                      (N_SM * ln * 2 * 1.965e9)}
-    extra["apply_N4096"] = ap
-    # timesteps/s for every config
-    cfgs = {}
-    for name, mk, pr, nst in (("C1_N16_f64", inputs.config1, ds.F64, 10_000),
-                              ("C2_N128_f32", inputs.config2, ds.F32, 10_000),
-                              ("C2_N128_f64", inputs.config2, ds.F64, 10_000),
-                              ("C3_N1024_f32", inputs.config3, ds.F32, 10_000),
-                              ("C4_N4096_f32", inputs.config4, ds.F32, 1000),
-                              ("C4_N4096_f64", inputs.config4, ds.F64, 1000),
-                              ("C5_B64_N512_f32", inputs.config5, ds.F32, 2000)):
-        wc = w if mk is inputs.config4 else mk()
-        t, _ = time_steps(torch, ds, wc, pr, ds.RPY, nst, 64)
-        cfgs[name] = {"timesteps_per_s": nst / t, "pairs_per_s": nst * 2 * pairs_per_apply(wc.N, wc.B) / t,
-                      "steps_timed": nst}
-    extra["configs_rpy_heun"] = cfgs
-    # the stroke-averaged far-field model (Eq. 9), the paper's comparison system: one right-hand side (S^2 dumbbell pairs)
+def avg_model_extra(torch, ds, sizes=(729, 2048, 8192)):
+    """The stroke-averaged far-field model (Eq. 9): one right-hand side (S^2 dumbbell pairs) and one
+    Heun step at the paper's largest S = 729 and two larger sizes."""
     avg = {}
-    for S_ in (729, 2048, 8192):
+    for S_ in sizes:
         rng = np.random.default_rng(S_)
         Rr = torch.as_tensor(rng.uniform(-200, 200, (S_, 3)).astype(np.float32), device="cuda")
         Nr = rng.standard_normal((S_, 3)); Nr /= np.linalg.norm(Nr, axis=1, keepdims=True)
@@ -366,7 +339,39 @@ def extras(torch, ds, inputs, w, args, precision, tensor):
                          "note": "ds_avg_rhs on device buffers (sin/cos table kernel + pair kernel per call) and ds_avg_step "
                                  "(2 launches per Heun step, FP64 state); FP32 pair arithmetic, 32 dumbbells x 8 slices per "
                                  "CTA, clusters of <= 8 CTAs per block of dumbbells"}
-    extra["avg_model_eq9"] = avg
+    return avg
+
+
+def extras(torch, ds, inputs, w, args, precision, tensor):
+    """Beside the headline: the standalone apply at N = 4096 (4 variants), timesteps/s of every config,
+    the cold-L2 per-step figure, and (with --sweep) the N = 256 .. 65536 apply sweep."""
+    extra = {}
+    # apply at N = 4096, all four variants (the standalone sweep of config 4)
+    Xa, Fa = inputs.apply_case(4096, 1004, 2004)
+    ap = {}
+    for pname, pr in (("f32", ds.F32), ("f64", ds.F64)):
+        for tname, tn in (("oseen", ds.OSEEN), ("rpy", ds.RPY)):
+            t = time_apply(torch, ds, 4096, pr, tn, Xa, Fa, reps=200)
+            ln = F32_LANES if pname == "f32" else F64_LANES
+            ap[f"{pname}_{tname}"] = {"us": t * 1e6, "pairs_per_s": pairs_per_apply(4096) / t,
+                                      "frac_of_alu_peak": pairs_per_apply(4096) * FLOP_PER_PAIR[tname] / t /
+                                      (N_SM * ln * 2 * 1.965e9)}
+    extra["apply_N4096"] = ap
+    # timesteps/s for every config
+    cfgs = {}
+    for name, mk, pr, nst in (("C1_N16_f64", inputs.config1, ds.F64, 10_000),
+                              ("C2_N128_f32", inputs.config2, ds.F32, 10_000),
+                              ("C2_N128_f64", inputs.config2, ds.F64, 10_000),
+                              ("C3_N1024_f32", inputs.config3, ds.F32, 10_000),
+                              ("C4_N4096_f32", inputs.config4, ds.F32, 1000),
+                              ("C4_N4096_f64", inputs.config4, ds.F64, 1000),
+                              ("C5_B64_N512_f32", inputs.config5, ds.F32, 2000)):
+        wc = w if mk is inputs.config4 else mk()
+        t, _ = time_steps(torch, ds, wc, pr, ds.RPY, nst, 64)
+        cfgs[name] = {"timesteps_per_s": nst / t, "pairs_per_s": nst * 2 * pairs_per_apply(wc.N, wc.B) / t,
+                      "steps_timed": nst}
+    extra["configs_rpy_heun"] = cfgs
+    extra["avg_model_eq9"] = avg_model_extra(torch, ds)
     extra["cold_l2"] = {"ms_per_step": 1e3 * time_steps_cold_l2(torch, ds, w, precision, tensor, 30),
                         "steps": 30, "flush": "512 MiB fill before every step"}
     if args.sweep:
@@ -477,6 +482,8 @@ def main():
     ap.add_argument("--cpu-steps", type=int, default=20, help="oracle Heun steps timed for cpu_baseline")
     ap.add_argument("--sweep", action="store_true", help="add the N = 256 .. 65536 apply sweep to extra")
     ap.add_argument("--quick", action="store_true", help="headline + e2e only (used under ncu)")
+    ap.add_argument("--avg-model", action="store_true",
+                    help="only the averaged-model timing of extra.avg_model_eq9 at S = 729 (used under ncu)")
     args = ap.parse_args()
     ref = args.impl == "reference"
     if args.steps is None:
@@ -489,6 +496,11 @@ def main():
         class _R:
             rank = int(os.environ.get("RANK", "0"))
         run_reference(args, _R())
+        return
+    if args.avg_model:
+        import torch
+        from paper_1004_1932_b200 import ds
+        print(json.dumps({"avg_model_eq9": avg_model_extra(torch, ds, sizes=(729,))}), flush=True)
         return
     ranks = Ranks()
     if ranks.world != args.gpus:

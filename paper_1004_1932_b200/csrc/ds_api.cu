@@ -386,7 +386,7 @@ int avg_sincos(ds_system *s, const double *dphi, int S) {
 template <typename T, typename IO>
 int launch_avg_rhs_t(ds_system *s, const IO *R, const IO *N, int S, IO *dR, IO *dN, const ds::AvgUpdate &U) {
     auto kern = ds::avg_rhs_kernel<T, IO>;
-    const int X = (S + ds::AVG_SB - 1) / ds::AVG_SB, slots = 4 * s->num_sms;
+    const int X = (S + ds::AVG_SB - 1) / ds::AVG_SB, slots = 2 * s->num_sms;   // two 512-thread CTAs per SM
     int Y = std::max(1, std::min(std::min(slots / X, ds::AVG_YMAX), (S + ds::AVG_W - 1) / ds::AVG_W));
     int chunk = (S + Y - 1) / Y;
     chunk = (chunk + ds::AVG_W - 1) / ds::AVG_W * ds::AVG_W;
