@@ -229,7 +229,7 @@ def test_batch_step_config5_three_systems():
 @pytest.mark.parametrize("tensor", [ds.OSEEN, ds.RPY])
 def test_step_integrators_tensors_chunking_t0(integrator, tensor):
     """Euler and Heun, both tensors, t0 != 0, odd step counts; the result does not depend on how the
-    steps are split over calls (graph replays vs single launches), bit for bit."""
+    steps are split over calls (one persistent launch vs several), bit for bit."""
     w = inputs.config2()
     Xa, X0, p = gpu_steps(w, ds.F64, 101, tensor, integrator, t0=0.25)
     Xb, _, _ = gpu_steps(w, ds.F64, 101, tensor, integrator, t0=0.25, chunks=[1, 33, 3, 64])
