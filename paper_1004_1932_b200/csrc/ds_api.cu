@@ -118,6 +118,7 @@ size_t elem_size(const ds_system *s) { return s->P.precision == DS_F64 ? sizeof(
 // Launch shape of the stateless apply: n_cta row tiles (mobility.cuh), any number of waves.  Every CTA
 // walks all U units with n_jg = NT / nq beta-groups, i.e. ceil(U / n_jg) iterations of 4 alpha x 1 unit
 // per thread, so the modelled time is waves x (iterations + a fixed per-CTA cost, in iterations).
+constexpr double ROW_COST = 0.4;   // cost of one more quad of rows in a CTA's tail, in pair-loop iterations
 int choose_tiles_apply(const ds_system *s, int NQ, int U) {
     const int lo = (NQ + ds::NT - 1) / ds::NT;  // nq <= NT
     if (s->tune_cta > 0) {
@@ -132,7 +133,7 @@ int choose_tiles_apply(const ds_system *s, int NQ, int U) {
         const int n_jg = ds::NT / nq;
         const long long iters = (U + n_jg - 1) / n_jg;
         const long long waves = ((long long)n + s->num_sms - 1) / s->num_sms;
-        const double cost = (double)waves * ((double)iters + 6.0);
+        const double cost = (double)waves * ((double)iters + 6.0 + ROW_COST * nq);
         if (cost < best_cost * (1.0 - 1e-9)) { best_cost = cost; best = n; }
     }
     return best;
@@ -157,7 +158,10 @@ int choose_shape_step(ds_system *s) {
             int per = s->num_sms / n;
             per = per < 1 ? 1 : (per > s->B ? s->B : per);
             const long long groups = (s->B + per - 1) / per;
-            const double cost = (double)groups * ((double)iters + (n > 1 ? 6.0 : 4.0));   // a stage's fixed part, in iterations: barrier + hand-over / local
+            // a stage's fixed part, in iterations: barrier + hand-over / local, and the tail (reduction, integrator,
+            // Eq. (4)), which grows with the rows a CTA owns: at equal iterations more CTAs win (measured, N = 128:
+            // 3.0 us per stage on 32 CTAs against 3.9 on 4)
+            const double cost = (double)groups * ((double)iters + (n > 1 ? 6.0 : 4.0) + ROW_COST * nq);
             if (cost < best_cost * (1.0 - 1e-9)) { best_cost = cost; best = n; }
         }
     }
