@@ -147,7 +147,9 @@ int ds_msd(ds_system *s, double *msd);
  * [S] double; device or host pointers.
  *   ds_avg_rhs : dR = sum_r J^{sr},  dN = -(1 - N N) sum_r K^{sr}   (right-hand sides of (9a), (9b)).
  *   ds_avg_step: n_steps Heun steps of size dt on R, Nv in place; the state is FP64 inside the call (the
- *                increments are below FP32 resolution) and Nv is renormalised after every stage.      */
+ *                increments are below FP32 resolution) and Nv is renormalised after every stage.
+ * Precondition, not checked: distinct centres (Eq. (9) is a far-field expansion, |R^s - R^r| >> ell; a pair at zero
+ * distance is skipped like the self term).                                                                        */
 int ds_avg_rhs(ds_system *s, const void *R, const void *Nv, const void *phase, void *dR, void *dN, int32_t S);
 int ds_avg_step(ds_system *s, void *R, void *Nv, const void *phase, int32_t S, double dt, int64_t n_steps);
 
