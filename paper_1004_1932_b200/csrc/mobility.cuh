@@ -418,9 +418,13 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
     // 48-byte thread stride: conflict-free); the sums of quad ith are elements 12 ith + m of the CTA's state.
     // A task = (quad ith, 4 consecutive m) is summed by RP consecutive lanes: lane part adds the groups
     // jg = part, part + RP, ... with one LDS.128 each, then log2(RP) shuffle steps.
-    const int rp_log = n_jg >= 32 ? 3 : (n_jg >= 16 ? 2 : (n_jg >= 8 ? 1 : 0));   // few groups: fewer lanes per task, more tasks per pass
-    const int RP = 1 << rp_log, tpw = 32 >> rp_log;                              // lanes per task, tasks per warp
     const int n_task = 3 * nq;                                  // tasks of the CTA
+    // few groups: fewer lanes per task, more tasks per pass; many groups and few tasks (small systems spread over many
+    // CTAs): up to a warp per task while a lane would otherwise add more than 8 groups and every task still gets its
+    // lanes in one pass (N = 4096 on 147 CTAs, 73 groups, stays at 8 lanes: wider measured no gain there)
+    int rp_log = n_jg >= 32 ? 3 : (n_jg >= 16 ? 2 : (n_jg >= 8 ? 1 : 0));
+    while (rp_log < 5 && n_jg >= (16 << rp_log) && (n_task << (rp_log + 1)) <= NT) ++rp_log;
+    const int RP = 1 << rp_log, tpw = 32 >> rp_log;                              // lanes per task, tasks per warp
     const int my_task = tid >> rp_log, my_part = tid & (RP - 1);
     if (tid == 0) {
         for (int s = 0; s < NS_MAX; ++s) {
@@ -771,7 +775,7 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
                 }
                 DS_PROBE(18);
 #pragma unroll
-                for (int d = 1; d < 8; d <<= 1) {
+                for (int d = 1; d < 32; d <<= 1) {
                     if (d < RP) {   // CTA-uniform
                         s0 += __shfl_xor_sync(0xffffffffu, s0, d); s1 += __shfl_xor_sync(0xffffffffu, s1, d);
                         s2 += __shfl_xor_sync(0xffffffffu, s2, d); s3 += __shfl_xor_sync(0xffffffffu, s3, d);
