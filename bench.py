@@ -425,7 +425,7 @@ def run_ours(args, ranks):
         roof = {"bound": "alu", "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s",
                 "frac": achieved / peak_nominal, "traffic": None,
                 "traffic_note": "ALU-bound path: DRAM bytes of the whole 50-step launch by ncu --set full are 0.37 MB "
-                                "(profiles/r1e_run_kernel_ncu_full.md); the algorithmic traffic is the 96 KB L2-resident "
+                                "(profiles/r1g_run_kernel_ncu_full.md); the algorithmic traffic is the 96 KB L2-resident "
                                 "stream read by each CTA per stage",
                 "kernel": "ds::run_kernel<float|double, tensor> (persistent: per stage pair sum + split-beta reduce + "
                           "Eq. (3a) + Heun update + Eq. (4) + inter-CTA barrier; ONE launch for all timed steps)",
