@@ -303,6 +303,9 @@ def workload_config(w, args, dtype):
                   "(512 MiB flush before every step) is in extra.cold_l2"}
 
 
+AVG_FLOP_PER_PAIR = 93
+
+
 def avg_model_extra(torch, ds, sizes=(729, 2048, 8192)):
     """The stroke-averaged far-field model (Eq. 9): one right-hand side (S^2 dumbbell pairs) and one
     Heun step at the paper's largest S = 729 and two larger sizes."""
@@ -336,6 +339,9 @@ def avg_model_extra(torch, ds, sizes=(729, 2048, 8192)):
             ts = e0.elapsed_time(e1) * 1e-3 / nst
         avg[f"S{S_}"] = {"us_per_rhs": t * 1e6, "dumbbell_pairs_per_s": S_ * (S_ - 1) / t,
                          "us_per_heun_step": ts * 1e6, "dumbbell_pairs_per_s_stepping": 2 * S_ * (S_ - 1) / ts,
+                         # 93 FLOP per ordered dumbbell pair of Eq. (9c,d) as the kernel evaluates it (FMA = 2)
+                         "flop_per_pair": AVG_FLOP_PER_PAIR,
+                         "frac_of_alu_peak_stepping": 2 * S_ * (S_ - 1) * AVG_FLOP_PER_PAIR / ts / (N_SM * F32_LANES * 2 * 1.965e9),
                          "note": "ds_avg_rhs on device buffers (sin/cos table kernel + pair kernel per call) and ds_avg_step "
                                  "(2 launches per Heun step, FP64 state); FP32 pair arithmetic, 32 dumbbells x 8 slices per "
                                  "CTA, clusters of <= 8 CTAs per block of dumbbells"}
