@@ -33,8 +33,9 @@
  *   R9  one radius a for all spheres.
  *
  * Parity pins: every function here is pinned by tests/test_oracle_pins.py against closed
- * forms, textbook series and invariants (P1-P10 of SURVEY.md 8(c)); nothing is "parity
- * unpinned".
+ * forms, textbook series, published known answers and invariants (P1-P10 of SURVEY.md 8(c),
+ * P11-P22 for the functions added since: the table in DESIGN.md section 3 lists them function
+ * by function); nothing is "parity unpinned".  (A comment only: no arithmetic changed.)
  *
  * Storage: 0-based; dumbbell s owns spheres 2s and 2s+1 (paper, 1-based: 2s-1 and 2s,
  * PAPER.md:63).  X, F, u are [N][3] row-major doubles, N = 2S.

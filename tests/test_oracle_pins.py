@@ -582,3 +582,94 @@ def test_P20_averaged_model_matches_the_microscopic_one_in_the_far_field():
     Rs, Ns = oracle.avg_step(Ra, Na, phi, 0.5, 2 * periods, p)
     assert np.linalg.norm((Rs - Ra)[0] - (Rb - Ra)[0]) <= 0.04 * np.linalg.norm((Rb - Ra)[0])
     np.testing.assert_allclose(np.linalg.norm(Ns, axis=1), 1.0, rtol=0, atol=1e-15)
+
+
+# --------------------------------------------------------------------------------- P21, P22: the two integrators
+def _avg_case():
+    """Three non-aligned dumbbells two to three lengths apart: the directions turn by tens of degrees over the test."""
+    R = np.array([[0.0, 0.0, 0.0], [22.0, 3.0, -2.0], [5.0, 24.0, 6.0]])
+    N = np.array([[1.0, 0.6, 0.0], [0.3, 1.0, 0.2], [-0.5, 0.2, 1.0]])
+    N /= np.linalg.norm(N, axis=1, keepdims=True)
+    return R, N, np.array([0.0, np.pi / 2, 2.2])
+
+
+def test_P21_averaged_model_integrator_is_second_order_heun():
+    """PAPER.md:236 and reading R16: Eq. (9) is stepped with the one-step Heun predictor-corrector, N
+    renormalised after the predictor and after the corrector.  (a) Order: against a reference at dt/256 the error at
+    dt, dt/2, dt/4, dt/8 falls by about 4 per halving (a plain-Euler corrector gives about 2 and fails).  (b) One step
+    rebuilt from the already pinned right-hand side (P18-P20): R + dt/2 (f(R, N) + f(R*, N*/|N*|)), N likewise and
+    normalised, equals avg_step to rounding; leaving out either renormalisation, or the corrector, is far outside."""
+    p = oracle.Params()
+    R, N, phi = _avg_case()
+    T_end = 4000.0
+    Rr, Nr = oracle.avg_step(R, N, phi, T_end / 4096, 4096, p)
+    turn = np.degrees(np.arccos(np.clip(np.sum(N * Nr, axis=1), -1, 1)))
+    assert turn.max() > 30.0                       # N turns visibly: the (9b) part of the integrator is exercised
+    eR, eN = [], []
+    for n in (16, 32, 64, 128):
+        Rn, Nn = oracle.avg_step(R, N, phi, T_end / n, n, p)
+        eR.append(np.abs(Rn - Rr).max()); eN.append(np.abs(Nn - Nr).max())
+    for e in (eR, eN):
+        ratios = [e[i] / e[i + 1] for i in range(3)]
+        assert all(3.6 < r < 4.4 for r in ratios), ratios
+    # (b) one large step from pinned parts
+    dt = 250.0
+    unit = lambda v: v / np.linalg.norm(v, axis=1, keepdims=True)
+
+    def one_step(renorm_pred=True, renorm_end=True, corrector=True):
+        dR1, dN1 = oracle.avg_rhs(R, N, phi, p)
+        Rp, Np = R + dt * dR1, N + dt * dN1
+        if renorm_pred:
+            Np = unit(Np)
+        if not corrector:
+            return Rp, unit(Np)
+        dR2, dN2 = oracle.avg_rhs(Rp, Np, phi, p)
+        R1, N1 = R + 0.5 * dt * (dR1 + dR2), N + 0.5 * dt * (dN1 + dN2)
+        return R1, (unit(N1) if renorm_end else N1)
+
+    Ro, No = oracle.avg_step(R, N, phi, dt, 1, p)
+    Ra, Na = one_step()
+    np.testing.assert_allclose(Ra, Ro, rtol=0, atol=1e-13)
+    np.testing.assert_allclose(Na, No, rtol=0, atol=1e-15)
+    np.testing.assert_allclose(np.linalg.norm(No, axis=1), 1.0, rtol=0, atol=1e-15)
+    for kw in (dict(renorm_pred=False), dict(renorm_end=False), dict(corrector=False)):
+        Rb, Nb = one_step(**kw)
+        assert max(np.abs(Rb - Ro).max(), np.abs(Nb - No).max()) > 1e-6, kw      # the pin tells these readings apart
+    # two steps in one call = two calls of one step (no hidden state)
+    R2, N2 = oracle.avg_step(R, N, phi, dt, 2, p)
+    R2b, N2b = oracle.avg_step(Ro, No, phi, dt, 1, p)
+    assert np.array_equal(R2, R2b) and np.array_equal(N2, N2b)
+
+
+@pytest.mark.parametrize("tensor", [OSEEN, RPY])
+def test_P22_heun_with_additive_noise_shares_the_increment(tensor):
+    """PAPER.md:236 ("can easily incorporate additive noise"), reading R15: with k_B T > 0 one increment
+    dW per step enters the predictor AND the corrector:
+        X* = X + dt V(X, t_n) + dW,   X_{n+1} = X + dt/2 (V(X, t_n) + V(X*, t_{n+1})) + dW.
+    Three steps rebuilt from the pinned parts (oracle.velocity: P1-P8; oracle.noise_normal: P14, P15) equal oracle.step
+    to rounding; a predictor without dW, a corrector evaluated at t_n, or increments drawn with the wrong step index
+    are far outside (the increments are ~ 2e-3, the readings differ by ~ 1e-4)."""
+    kT, seed, system, t0 = 0.05, 11, 2, 0.3
+    p = oracle.Params(kT=kT, seed=seed, system=system, tensor=tensor)
+    X0, phase = inputs.random_suspension(2, 5, side=30.0)
+    dt = p.dt
+    amp = np.sqrt(2 * kT * dt / (6 * np.pi * p.eta * p.a))
+
+    def rebuild(pred_noise=True, t_corr_shift=1, index_shift=0):
+        X = X0.copy()
+        for n in range(3):
+            dW = amp * np.array([oracle.noise_normal(seed, n + index_shift, system, k) for k in range(X.size)]).reshape(X.shape)
+            V1 = oracle.velocity(X, phase, t0 + n * dt, p)
+            Xp = X + dt * V1 + (dW if pred_noise else 0.0)
+            V2 = oracle.velocity(Xp, phase, t0 + (n + t_corr_shift) * dt, p)
+            X = X + 0.5 * dt * (V1 + V2) + dW
+        return X
+
+    Xo = oracle.step(X0, phase, t0, 0, 3, p)
+    np.testing.assert_allclose(rebuild(), Xo, rtol=0, atol=1e-13)
+    assert np.abs(rebuild(pred_noise=False) - Xo).max() > 1e-5
+    assert np.abs(rebuild(t_corr_shift=0) - Xo).max() > 1e-7
+    assert np.abs(rebuild(index_shift=1) - Xo).max() > 1e-4
+    # steps 1..2 of a run that starts at n_done = 1 use the increments of steps 1 and 2 (counter = absolute step index)
+    X1 = oracle.step(X0, phase, t0, 0, 1, p)
+    assert np.array_equal(oracle.step(X1, phase, t0, 1, 2, p), Xo)
