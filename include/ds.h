@@ -22,10 +22,13 @@
  *   Every data pointer may be a DEVICE pointer (e.g. a torch tensor's data_ptr()) or a HOST
  *   pointer (pageable or pinned); the library asks the CUDA runtime which (cudaPointerGetAttributes)
  *   and stages host buffers through its own device scratch with cudaMemcpyAsync on the system's
- *   stream.  The caller owns all buffers; the library never keeps a caller pointer past the call.
+ *   stream.  The caller owns all buffers; the library never stores a caller pointer in the system.
  *   Work is enqueued on the system's stream.  Calls with device pointers are asynchronous; calls
- *   that write to a HOST pointer synchronise the stream before returning.  ds_create/ds_destroy
- *   are synchronous.
+ *   that write to a HOST pointer synchronise the stream before returning.  Calls that only READ
+ *   host pointers do not synchronise: a pageable input has been staged when the call returns, but
+ *   a PINNED host input is read by the copy engine when the stream reaches the copy, so it must
+ *   stay unchanged until then (until the next synchronising call on the system, or a
+ *   cudaStreamSynchronize of its stream).  ds_create/ds_destroy are synchronous.
  *
  * Errors
  *   Every call returns DS_OK (0) or a negative ds_status; nothing throws across the ABI.
@@ -46,6 +49,8 @@ extern "C" {
 #endif
 
 typedef struct ds_system ds_system; /* opaque; owned by the library, freed by ds_destroy */
+
+#define DS_MAX_APPLY_N (1 << 28)     /* largest n of ds_mobility_apply (the kernel indexes 16-byte pieces of the stream in 32 bits) */
 
 enum { DS_F32 = 0, DS_F64 = 1 };     /* element type of user buffers and of the O(N^2) pair arithmetic */
 enum { DS_OSEEN = 0, DS_RPY = 1 };   /* Eq. (3b): first line only / both lines */
@@ -92,7 +97,9 @@ int ds_create(const ds_params *p, ds_system **out);
 /* Free everything the system owns.  Synchronises the system's stream first.  NULL is a no-op. */
 int ds_destroy(ds_system *s);
 
-/* Re-target the system to another cudaStream_t (e.g. one that is being captured). */
+/* Re-target the system to another cudaStream_t (e.g. one that is being captured).  Work already queued on the old
+ * stream is ordered before anything enqueued on the new one (an event); if the OLD stream is being captured at the
+ * time of the call, the caller owns that ordering. */
 int ds_set_stream(ds_system *s, void *stream);
 
 /* Set the state: sphere positions pos [B][N][3] (user precision), stroke phases phase [B][S]
@@ -111,8 +118,8 @@ int ds_forces(ds_system *s, void *F);
 /* Stateless mobility apply, Eq. (1a) deterministic part with Eq. (3a,3b), PAPER.md:38, 57-59:
  *   u_a = F_a / (6 pi eta a) + sum_{b != a} T(x_a - x_b) F_b,   a = 0 .. n-1,
  *   Oseen: T(r) = 1/(8 pi eta r) (1 + rr/r^2);  RPY: + 2a^2/(24 pi eta r^3) (1 - 3 rr/r^2).
- * pos, F, u are [n][3] in user precision; n >= 1 is any sphere count (odd allowed, independent of
- * S); a, eta, tensor and precision come from the system.  u must not alias pos or F.
+ * pos, F, u are [n][3] in user precision; 1 <= n <= DS_MAX_APPLY_N is any sphere count (odd allowed,
+ * independent of S; DS_ERR_INVALID_PARAM outside that range); a, eta, tensor and precision come from the system.  u must not alias pos or F.
  * Does not touch the system's state.                                                           */
 int ds_mobility_apply(ds_system *s, const void *pos, const void *F, void *u, int32_t n);
 
@@ -152,23 +159,6 @@ int ds_msd(ds_system *s, double *msd);
  * distance is skipped like the self term).                                                                        */
 int ds_avg_rhs(ds_system *s, const void *R, const void *Nv, const void *phase, void *dR, void *dN, int32_t S);
 int ds_avg_step(ds_system *s, void *R, void *Nv, const void *phase, int32_t S, double dt, int64_t n_steps);
-
-/* Launch-shape override for tuning and tests: number of row tiles (CTAs) per system; 0 = library
- * heuristic.  Values below ceil(ceil(N/4)/512) or above ceil(N/4) are clamped; the step modes also
- * clamp to the SM count (their CTAs meet at a barrier every stage and must be co-resident).      */
-int ds_set_tuning(ds_system *s, int32_t n_tiles);
-
-/* Development instrumentation: device_buffer (DEVICE pointer, 16 int64 per CTA of the largest launch,
- * or NULL to switch off) receives clock64() samples of the last stage of every hot-kernel launch.  */
-int ds_set_probe(ds_system *s, void *device_buffer);
-
-/* Number of kernels launched by this system since creation (bench.py's gpu_launches claim). */
-int64_t ds_launch_count(const ds_system *s);
-
-/* Measurement aid for the roofline denominators (bench.py): runs an FMA-chain microbenchmark on
- * `device` (packed FP32 FMA for DS_F32, DFMA for DS_F64) and writes the best achieved FLOP/s
- * (FMA = 2) to *flops_per_s (HOST pointer).  Synchronous; uses the legacy default stream.       */
-int ds_peak_probe(int32_t precision, int32_t device, double *flops_per_s);
 
 const char *ds_strerror(int code);
 const char *ds_last_cuda_error(void); /* text of the last failing CUDA call on this thread, or "" */

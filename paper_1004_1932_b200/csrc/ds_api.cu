@@ -8,11 +8,14 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <mutex>
 #include <new>
 #include <vector>
 
 #include "../../include/ds.h"
+#include "../../include/ds_dev.h"
 #include "mobility.cuh"
+#include "pipeline.cuh"
 #include "peak.cuh"
 #include "averaged.cuh"
 #include "state.cuh"
@@ -39,6 +42,20 @@ thread_local char g_cuda_err[512] = "";
     } while (0)
 
 template <typename T> constexpr int pack_w() { return ds::Pack<T>::W; }
+
+// The opt-in to more than 48 KB of dynamic shared memory is a per-device attribute of a kernel: one instance of this
+// per kernel variant remembers on which devices it has been set (a mutex makes it safe for concurrent host threads).
+struct SmemOptIn {
+    std::mutex mu;
+    uint64_t done[4] = {0, 0, 0, 0};   // devices 0 .. 255
+    int ensure(const void *kern, int device) {
+        std::lock_guard<std::mutex> lock(mu);
+        if (device >= 0 && device < 256 && (done[device >> 6] >> (device & 63) & 1ULL)) return DS_OK;
+        CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, ds::SMEM_MAX));
+        if (device >= 0 && device < 256) done[device >> 6] |= 1ULL << (device & 63);
+        return DS_OK;
+    }
+};
 
 struct Buf {
     void *p = nullptr;
@@ -79,6 +96,16 @@ struct ds_system {
     unsigned int ll_tag = 1;                    // next unused tag (0 = never written)
     double *Xcg = nullptr, *V1g = nullptr, *Fg = nullptr, *Lg = nullptr;  // only when !state_smem
     long long *probe = nullptr;                 // caller's device buffer (ds_set_probe) or NULL
+    // pipelined step kernel (pipeline.cuh): used for ds_step / ds_batch_step when the shape allows it and the pair loop
+    // dominates a stage
+    int pipe_mode = -1;                         // -1 = library heuristic, 0 = never, 1 = whenever the shape allows it
+    bool use_pipe = false;
+    int *half_off = nullptr;                    // device table [2][n_cta + 1]
+    int half_off_cap = 0;
+    int reg_units[2] = {0, 0}, pbuf_units[2] = {0, 0}, rows_max = 0;
+    size_t pipe_smem = 0;
+    unsigned long long *pcnt = nullptr;         // [B][2] arrival counters of the two stream regions
+    unsigned long long pcnt_base = 0;
     // scratch of the stateless apply and of host-pointer staging
     Buf ap_units, st_a, st_b, st_c;
     Buf avg;                                    // FP64 scratch of the stroke-averaged model (Eq. 9)
@@ -198,11 +225,8 @@ bool stream_resident(int NQ, int U, int n_cta, int buf_bytes) {
 template <typename T, int TENSOR, int MODE, bool RES>
 int launch_run_v(ds_system *s, ds::RunArgs &A, dim3 grid, size_t smem, bool coop, cudaStream_t st) {
     auto kern = ds::run_kernel<T, TENSOR, MODE, RES>;
-    static bool attr_done = false;
-    if (!attr_done) {
-        CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, ds::SMEM_MAX));
-        attr_done = true;
-    }
+    static SmemOptIn opt_in;
+    DS_TRY(opt_in.ensure((const void *)kern, s->P.device));
     if (coop) {
         void *args[] = {(void *)&A};
         CU_TRY(cudaLaunchCooperativeKernel((const void *)kern, grid, dim3(ds::NT), args, smem, st));
@@ -262,6 +286,114 @@ void fill_constants(const ds_system *s, ds::RunArgs &A) {
     A.t0 = s->t0; A.dt = s->P.dt; A.ell = s->P.ell; A.lambda = s->P.lambda; A.omega = s->P.omega; A.k0 = s->P.k0;
     A.noise_amp = s->P.kT > 0.0 ? sqrt(2.0 * s->P.kT * s->P.dt * A.self_mob) : 0.0;   // Eq. (1a) with 2H ~ 2/(6 pi mu a) = C C^T
     A.seed = s->P.seed;
+}
+
+
+// Pipelined step kernel (pipeline.cuh): every CTA's rows are cut into two halves of whole quads; region h of a stream
+// holds the half-h units of all CTAs.  Builds the offset table and decides whether the shape is eligible: both halves
+// of every CTA at most 16 quads (one warp per quad at least), everything in shared memory.
+int setup_pipe(ds_system *s) {
+    s->use_pipe = false;
+    if (s->n_cta < 2 || s->pipe_mode == 0) return DS_OK;
+    const int n = s->n_cta, W = s->W;
+    std::vector<int> off(2 * (size_t)(n + 1), 0);
+    int rows_max = 0, nqh_max = 0;
+    std::vector<int> shapes;   // distinct beta-group counts n_jg = 32 (16 / nq_h) of all passes
+    for (int c = 0; c < n; ++c) {
+        const long long q0 = (long long)c * s->NQ / n, q1 = (long long)(c + 1) * s->NQ / n;
+        const int nq = (int)(q1 - q0);
+        const long long left = (long long)s->N - 4 * q0;
+        const int nrows = (int)(left < 4LL * nq ? left : 4LL * nq);
+        const int nqA = (nq + 1) / 2, nqB = nq - nqA;
+        const int rowsA = 4 * nqA < nrows ? 4 * nqA : nrows, rowsB = nrows - rowsA;
+        off[c + 1] = off[c] + rowsA / W;
+        off[(n + 1) + c + 1] = off[(n + 1) + c] + rowsB / W;
+        rows_max = nrows > rows_max ? nrows : rows_max;
+        nqh_max = nqA > nqh_max ? nqA : nqh_max;
+        for (int nqh : {nqA, nqB})
+            if (nqh > 0 && nqh <= ds::PIPE_CW) {   // the 16 warps of a pass: 16 / nqh per quad, or one more
+                shapes.push_back(32 * (ds::PIPE_CW / nqh));
+                if (ds::PIPE_CW % nqh) shapes.push_back(32 * (ds::PIPE_CW / nqh + 1));
+            }
+    }
+    if (nqh_max > ds::PIPE_CW) return DS_OK;
+    rows_max = (rows_max + 3) / 4 * 4;
+    int bu[2];
+    for (int h = 0; h < 2; ++h) {
+        const int U = off[(size_t)h * (n + 1) + n];
+        int cap = U;
+        for (int n_jg : shapes) { const int need = (U + n_jg - 1) / n_jg * n_jg; cap = need > cap ? need : cap; }
+        bu[h] = (cap + 7) / 8 * 8;
+    }
+    const size_t smem = (size_t)(bu[0] + bu[1]) * ds::UNIT_BYTES + ds::PIPE_BAR_BYTES + ds::PIPE_SCR_BYTES + ds::PIPE_TAB_BYTES +
+                       (size_t)rows_max * ds::STATE_BYTES_PER_ROW;
+    if (smem > (size_t)ds::SMEM_MAX) return DS_OK;
+    if (s->pipe_mode < 0) {
+        // heuristic: the pipeline hides a stage's fixed cost (about 5.5 k cycles) behind the pair loop of the other half;
+        // it pays once a quarter of a stage's pair work is longer than that: iterations of the unsplit shape >= 16
+        const int nq = (s->NQ + n - 1) / n, n_jg = ds::NT / nq;
+        if ((s->U + n_jg - 1) / n_jg < 16) return DS_OK;
+    }
+    if (s->half_off_cap < 2 * (n + 1)) {
+        if (s->half_off) CU_TRY(cudaFree(s->half_off));
+        s->half_off = nullptr; s->half_off_cap = 0;
+        CU_TRY(cudaMalloc((void **)&s->half_off, 2 * (size_t)(n + 1) * sizeof(int)));
+        s->half_off_cap = 2 * (n + 1);
+    }
+    CU_TRY(cudaMemcpy(s->half_off, off.data(), 2 * (size_t)(n + 1) * sizeof(int), cudaMemcpyHostToDevice));
+    s->reg_units[0] = off[n]; s->reg_units[1] = off[(size_t)(n + 1) + n];
+    s->pbuf_units[0] = bu[0]; s->pbuf_units[1] = bu[1];
+    s->rows_max = rows_max;
+    s->pipe_smem = smem;
+    s->use_pipe = true;
+    return DS_OK;
+}
+
+template <typename T, int TENSOR, bool HEUN>
+int launch_pipe_v(ds_system *s, ds::PipeArgs &A, dim3 grid) {
+    auto kern = ds::pipe_kernel<T, TENSOR, HEUN>;
+    static SmemOptIn opt_in;
+    DS_TRY(opt_in.ensure((const void *)kern, s->P.device));
+    void *args[] = {(void *)&A};
+    CU_TRY(cudaLaunchCooperativeKernel((const void *)kern, grid, dim3(ds::PIPE_NT), args, s->pipe_smem, s->stream));
+    s->launches += 1;
+    return DS_OK;
+}
+
+// RUN_STEP through the pipelined kernel: one launch per group of co-resident systems
+int launch_pipe_run(ds_system *s, long long n_steps) {
+    ds::PipeArgs A;
+    memset(&A, 0, sizeof A);
+    A.N = s->N; A.NQ = s->NQ; A.n_cta = s->n_cta; A.unit_stride = s->unit_stride;
+    A.units[0] = s->units[0]; A.units[1] = s->units[1];
+    A.half_off = s->half_off;
+    A.reg_units[0] = s->reg_units[0]; A.reg_units[1] = s->reg_units[1];
+    A.buf_units[0] = s->pbuf_units[0]; A.buf_units[1] = s->pbuf_units[1];
+    A.rows_max = s->rows_max;
+    ds::RunArgs R;
+    memset(&R, 0, sizeof R);
+    fill_constants(s, R);
+    A.self_mob = R.self_mob; A.pre = R.pre; A.c1 = R.c1; A.c2 = R.c2; A.c1f = R.c1f; A.c2f = R.c2f;
+    A.t0 = R.t0; A.dt = R.dt; A.ell = R.ell; A.lambda = R.lambda; A.omega = R.omega; A.k0 = R.k0;
+    A.noise_amp = R.noise_amp; A.seed = R.seed;
+    A.n0 = s->n_host; A.n_steps = n_steps;
+    A.X = s->X; A.xu = s->xu; A.from_user = s->x_valid ? 0 : 1; A.phase = s->phase;
+    A.cnt = s->pcnt; A.cnt_base = s->pcnt_base;
+    A.probe = s->probe;
+    const bool heun = s->P.integrator == DS_HEUN, f64 = s->P.precision == DS_F64, rpy = s->P.tensor == DS_RPY;
+    const long long n_stage = n_steps * (heun ? 2 : 1);
+    for (int b0 = 0; b0 < s->B; b0 += s->sys_per_launch) {
+        const int nb = s->B - b0 < s->sys_per_launch ? s->B - b0 : s->sys_per_launch;
+        A.b0 = b0;
+        const dim3 grid((unsigned)s->n_cta, (unsigned)nb);
+#define DS_PIPE(TT, TEN) (heun ? launch_pipe_v<TT, TEN, true>(s, A, grid) : launch_pipe_v<TT, TEN, false>(s, A, grid))
+        if (f64) DS_TRY(rpy ? DS_PIPE(double, ds::TENSOR_RPY) : DS_PIPE(double, ds::TENSOR_OSEEN));
+        else DS_TRY(rpy ? DS_PIPE(float, ds::TENSOR_RPY) : DS_PIPE(float, ds::TENSOR_OSEEN));
+#undef DS_PIPE
+    }
+    s->pcnt_base += (unsigned long long)s->n_cta * (unsigned long long)n_stage;
+    s->x_valid = true; s->xu_valid = true;
+    return DS_OK;
 }
 
 // RUN_VELOCITY (n_steps ignored) or RUN_STEP on the system's own state: one launch per group of
@@ -516,6 +648,8 @@ int ds_create(const ds_params *p, ds_system **out) {
     if (set_device(s) != DS_OK) return fail(DS_ERR_CUDA);
     rc = choose_shape_step(s);   // N too large for one co-resident grid: the step modes cannot run
     if (rc != DS_OK) return fail(rc);
+    rc = setup_pipe(s);
+    if (rc != DS_OK) return fail(rc);
     const size_t n3 = (size_t)s->B * s->N * 3;
     const size_t ub = (size_t)s->B * (size_t)s->unit_stride * ds::UNIT_BYTES;
     cudaError_t e = cudaSuccess;
@@ -526,11 +660,13 @@ int ds_create(const ds_params *p, ds_system **out) {
     al(&s->units[0], ub); al(&s->units[1], ub);
     al(&s->ll[0], 2 * ub); al(&s->ll[1], 2 * ub);
     al((void **)&s->bar, (size_t)s->B * sizeof(unsigned long long));
+    al((void **)&s->pcnt, 2 * (size_t)s->B * sizeof(unsigned long long));
     // global homes of the per-row state, used only by tiles too large for shared memory (any tuning)
     al((void **)&s->Xcg, n3 * 8); al((void **)&s->V1g, n3 * 8); al((void **)&s->Fg, n3 * 8);
     al((void **)&s->Lg, (size_t)s->B * s->S * 8);
     if (e != cudaSuccess) { snprintf(g_cuda_err, sizeof g_cuda_err, "cudaMalloc -> %s", cudaGetErrorString(e)); (void)cudaGetLastError(); return fail(DS_ERR_ALLOC); }
     if (cudaMemsetAsync(s->bar, 0, (size_t)s->B * sizeof(unsigned long long), s->stream) != cudaSuccess) return fail(DS_ERR_CUDA);
+    if (cudaMemsetAsync(s->pcnt, 0, 2 * (size_t)s->B * sizeof(unsigned long long), s->stream) != cudaSuccess) return fail(DS_ERR_CUDA);
     for (int k = 0; k < 2; ++k)
         if (cudaMemsetAsync(s->ll[k], 0, 2 * ub, s->stream) != cudaSuccess) return fail(DS_ERR_CUDA);
     for (int k = 0; k < 2 && rc == DS_OK; ++k) rc = f64 ? run_pad_init<double>(s, s->units[k]) : run_pad_init<float>(s, s->units[k]);
@@ -544,7 +680,7 @@ int ds_destroy(ds_system *s) {
     if (!s) return DS_OK;
     cudaSetDevice(s->P.device);
     cudaStreamSynchronize(s->stream);
-    void *ptrs[] = {s->X, s->xu, s->Rref, s->msd_part, s->msd_out, s->phase, s->units[0], s->units[1], s->ll[0], s->ll[1], s->bar, s->Xcg, s->V1g, s->Fg, s->Lg,
+    void *ptrs[] = {s->X, s->xu, s->Rref, s->msd_part, s->msd_out, s->phase, s->units[0], s->units[1], s->ll[0], s->ll[1], s->bar, s->pcnt, s->half_off, s->Xcg, s->V1g, s->Fg, s->Lg,
                     s->ap_units.p, s->st_a.p, s->st_b.p, s->st_c.p, s->avg.p, s->avg_sc.p};
     for (void *q : ptrs) if (q) cudaFree(q);
     (void)cudaGetLastError();
@@ -554,6 +690,18 @@ int ds_destroy(ds_system *s) {
 
 int ds_set_stream(ds_system *s, void *stream) {
     if (!s) return DS_ERR_NULL;
+    DS_TRY(set_device(s));
+    // work still queued on the old stream touches the system's buffers: the new stream waits for it.  While the old
+    // stream is being captured an event cannot order against it; the caller owns the ordering then.
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(s->stream, &cap) != cudaSuccess) { (void)cudaGetLastError(); cap = cudaStreamCaptureStatusNone; }
+    if (cap == cudaStreamCaptureStatusNone && (cudaStream_t)stream != s->stream) {
+        cudaEvent_t ev;
+        CU_TRY(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+        CU_TRY(cudaEventRecord(ev, s->stream));
+        CU_TRY(cudaStreamWaitEvent((cudaStream_t)stream, ev, 0));
+        CU_TRY(cudaEventDestroy(ev));
+    }
     s->stream = (cudaStream_t)stream;
     return DS_OK;
 }
@@ -564,8 +712,20 @@ int ds_set_tuning(ds_system *s, int32_t n_tiles) {
     DS_TRY(set_device(s));
     CU_TRY(cudaStreamSynchronize(s->stream));
     s->tune_cta = n_tiles;
-    return choose_shape_step(s);
+    DS_TRY(choose_shape_step(s));
+    return setup_pipe(s);
 }
+
+int ds_set_pipeline(ds_system *s, int32_t mode) {
+    if (!s) return DS_ERR_NULL;
+    if (mode < -1 || mode > 1) return DS_ERR_INVALID_PARAM;
+    DS_TRY(set_device(s));
+    CU_TRY(cudaStreamSynchronize(s->stream));
+    s->pipe_mode = mode;
+    return setup_pipe(s);
+}
+
+int ds_pipeline_active(const ds_system *s) { return s && s->use_pipe ? 1 : 0; }
 
 int ds_set_probe(ds_system *s, void *device_buffer) {
     if (!s) return DS_ERR_NULL;
@@ -788,7 +948,7 @@ int ds_velocity(ds_system *s, void *V) {
 
 int ds_mobility_apply(ds_system *s, const void *pos, const void *F, void *u, int32_t n) {
     if (!s || !pos || !F || !u) return DS_ERR_NULL;
-    if (n < 1) return DS_ERR_INVALID_PARAM;
+    if (n < 1 || n > DS_MAX_APPLY_N) return DS_ERR_INVALID_PARAM;   // the kernel's piece arithmetic is 32-bit
     DS_TRY(set_device(s));
     const bool f64 = s->P.precision == DS_F64;
     const size_t nb = (size_t)n * 3 * elem_size(s);
@@ -847,7 +1007,7 @@ int ds_batch_step(ds_system *s, int64_t n_steps) {
     int64_t left = n_steps;
     while (left > 0) {   // one launch runs up to MAX_STEPS_PER_LAUNCH steps entirely on the device
         const long long k = left < MAX_STEPS_PER_LAUNCH ? left : MAX_STEPS_PER_LAUNCH;
-        DS_TRY(launch_state_run(s, ds::RUN_STEP, k, nullptr));
+        DS_TRY(s->use_pipe ? launch_pipe_run(s, k) : launch_state_run(s, ds::RUN_STEP, k, nullptr));
         s->n_host += k; left -= k;
     }
     return DS_OK;

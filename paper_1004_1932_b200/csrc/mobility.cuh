@@ -785,7 +785,7 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
                 if (my_part != 0 || task >= n_task) continue;
                 // state elements e0 .. e0 + 3 of the CTA (e = 3 (local row) + component): Eq. (3a) and the
                 // 1/(8 pi mu) factor in FP64, then the integrator.  Straight-line: the four elements
-                // are independent and only the stores are predicated (the state arrays are padded to whole quads).
+                // are independent.
                 const int e0 = 4 * task;
                 const T sums[4] = {s0, s1, s2, s3};
                 if constexpr (!stepping) {               // RUN_APPLY: a2 + a3 with the stream's own F
@@ -799,9 +799,15 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
                         }
                     }
                 } else {
+                // the shared-memory state is padded to whole quads; its global home (state_smem == 0) is not: a last quad
+                // of two rows must neither read nor write past its system
+                const int e_end = A.state_smem ? e0 + 4 : 3 * nrows;
                 double v[4], xo[4], v1[4];
 #pragma unroll
-                for (int j = 0; j < 4; ++j) { v[j] = A.self_mob * Fs[e0 + j] + A.pre * (double)sums[j]; xo[j] = Xs[e0 + j]; v1[j] = V1s[e0 + j]; }
+                for (int j = 0; j < 4; ++j) {
+                    const bool in = e0 + j < e_end;
+                    v[j] = A.self_mob * (in ? Fs[e0 + j] : 0.0) + A.pre * (double)sums[j]; xo[j] = in ? Xs[e0 + j] : 0.0; v1[j] = in ? V1s[e0 + j] : 0.0;
+                }
                 if (MODE == KM_VELOCITY) {
 #pragma unroll
                     for (int j = 0; j < 4; ++j)
@@ -819,9 +825,11 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
                     const double w = corr ? v1[j] + v[j] : v[j];
                     double xn = xo[j] + cdt * w;
                     if (A.noise_amp != 0.0) xn += A.noise_amp * noise_normal(A.seed, nstep, b, 3 * r0 + e);
-                    if (pred) V1s[e] = v[j]; else Xs[e] = xn;
-                    Xc[e] = xn;
-                    if (XcT != nullptr) XcT[e] = (T)xn;
+                    if (e < e_end) {
+                        if (pred) V1s[e] = v[j]; else Xs[e] = xn;
+                        Xc[e] = xn;
+                        if (XcT != nullptr) XcT[e] = (T)xn;
+                    }
                 }
                 }
             }

@@ -22,8 +22,9 @@ ERR_INVALID_PARAM, ERR_NULL, ERR_CUDA, ERR_STATE, ERR_NO_DEVICE, ERR_ALLOC = -1,
 
 # every symbol include/ds.h declares (tests check that the built library exports all of them)
 SYMBOLS = ["ds_create", "ds_destroy", "ds_set_stream", "ds_set_state", "ds_get_state", "ds_forces",
-           "ds_mobility_apply", "ds_step", "ds_batch_step", "ds_velocity", "ds_dumbbell_coords", "ds_msd_set_reference", "ds_msd", "ds_avg_rhs", "ds_avg_step", "ds_set_tuning", "ds_set_probe", "ds_launch_count",
-           "ds_peak_probe", "ds_strerror", "ds_last_cuda_error", "ds_version"]
+           "ds_mobility_apply", "ds_step", "ds_batch_step", "ds_velocity", "ds_dumbbell_coords", "ds_msd_set_reference", "ds_msd", "ds_avg_rhs", "ds_avg_step", "ds_strerror", "ds_last_cuda_error", "ds_version"]
+# development / measurement hooks (include/ds_dev.h)
+DEV_SYMBOLS = ["ds_set_tuning", "ds_set_probe", "ds_launch_count", "ds_peak_probe", "ds_set_pipeline", "ds_pipeline_active"]
 
 
 class DsError(RuntimeError):
@@ -71,6 +72,8 @@ def lib():
         L.ds_msd.argtypes = [vp, ctypes.POINTER(dbl)]
         L.ds_set_tuning.argtypes = [vp, i32]
         L.ds_set_probe.argtypes = [vp, vp]
+        L.ds_set_pipeline.argtypes = [vp, i32]
+        L.ds_pipeline_active.argtypes = [vp]
         L.ds_launch_count.argtypes = [vp]
         L.ds_launch_count.restype = i64
         L.ds_peak_probe.argtypes = [i32, i32, ctypes.POINTER(dbl)]
@@ -189,6 +192,12 @@ class System:
 
     def set_tuning(self, n_tiles=0):
         _check(lib().ds_set_tuning(self._h, int(n_tiles)), "ds_set_tuning")
+
+    def set_pipeline(self, mode=-1):
+        _check(lib().ds_set_pipeline(self._h, int(mode)), "ds_set_pipeline")
+
+    def pipeline_active(self):
+        return bool(lib().ds_pipeline_active(self._h))
 
     def set_probe(self, buf=None):
         _check(lib().ds_set_probe(self._h, _ptr(buf)), "ds_set_probe")

@@ -11,8 +11,8 @@ from paper_1004_1932_b200 import ds
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def _declared_symbols():
-    src = open(os.path.join(ROOT, "include", "ds.h")).read()
+def _declared_symbols(header="ds.h"):
+    src = open(os.path.join(ROOT, "include", header)).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(ds_[a-z_0-9]+)\s*\(", src)))
 
@@ -24,6 +24,12 @@ def test_library_exports_every_declared_symbol():
     for name in declared:
         assert hasattr(L, name), f"{name} declared in include/ds.h but not exported by libds.so"
     assert sorted(ds.SYMBOLS) == declared
+    # the development hooks live in their own header (include/ds_dev.h), not in the product boundary
+    dev = _declared_symbols("ds_dev.h")
+    for name in dev:
+        assert hasattr(L, name), f"{name} declared in include/ds_dev.h but not exported by libds.so"
+    assert sorted(ds.DEV_SYMBOLS) == dev
+    assert not set(dev) & set(declared)
 
 
 def test_version_and_strerror():

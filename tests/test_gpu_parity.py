@@ -73,6 +73,8 @@ def test_apply_parity_sizes(N, tensor, precision):
     ref = oracle_apply(X, F, precision, tensor, a=0.9, eta=1.3)
     assert np.isfinite(u).all()
     assert rel_l2(u, ref) <= TOL[precision]
+    # per row: no single sphere is off by more than a few tolerances of the typical |u|
+    assert np.abs(u - ref).max() <= 20 * TOL[precision] * np.sqrt(np.mean(ref ** 2))
 
 
 @pytest.mark.parametrize("precision", [ds.F32, ds.F64])
@@ -616,3 +618,160 @@ def test_avg_step_parity_729(precision):
         assert np.abs(Rg - Ro).max() <= 1e-12 * 250 and np.abs(Ng - No).max() <= 1e-12
     else:   # float32 output buffers: half an ulp of 250 is 1.5e-5
         assert np.abs(Rg - Ro).max() <= 2e-5 and np.abs(Ng - No).max() <= 1e-5
+
+
+# --------------------------------------------------------------------------------- pipelined step kernel (pipeline.cuh)
+def pipe_steps(w, precision, chunks, n_tiles=0, tensor=ds.RPY, integrator=ds.HEUN, t0=0.0, pipeline=1, host=False, **kw):
+    """Steps through the two-pass pipelined kernel (forced on; `pipeline=0` forces the one-pass kernel)."""
+    s, p = make_system(w, precision, tensor, integrator, **kw)
+    with s:
+        if n_tiles:
+            s.set_tuning(n_tiles)
+        s.set_pipeline(pipeline)
+        assert s.pipeline_active() == bool(pipeline), (w.N, n_tiles)
+        X0 = rounded(w, precision)
+        if host:
+            s.set_state(np.ascontiguousarray(X0, dtype=NPDT[precision]), np.ascontiguousarray(w.phase), t0=t0)
+        else:
+            s.set_state(dev(X0, precision), torch.as_tensor(w.phase, device="cuda"), t0=t0)
+        for c in chunks:
+            s.batch_step(c) if w.B > 1 else s.step(c)
+        out = torch.empty((w.B, w.N, 3), dtype=TDT[precision], device="cuda")
+        s.get_state(out)
+        torch.cuda.synchronize()
+        return out.cpu().numpy().astype(np.float64), X0, p
+
+
+@pytest.mark.parametrize("precision,tol", [(ds.F32, 1e-4), (ds.F64, 1e-10)])
+@pytest.mark.parametrize("S,n_tiles", [(192, 3), (192, 17), (192, 48), (191, 5), (97, 2), (333, 31), (600, 148), (1024, 0)])
+def test_pipeline_parity_shapes(S, n_tiles, precision, tol):
+    """The pipelined kernel under forced row tilings: halves of 1 ... 16 quads (16 ... 1 warps per quad), CTAs with an
+    empty second half (48 tiles of N = 384: one quad each), odd S (a last quad of two rows), regions that end inside a
+    warp's 32 units, the library's own tiling (S = 1024: 128 CTAs).  50 Heun steps split over three launches, t0 != 0,
+    element by element against the oracle."""
+    w = inputs.config5(B=1, S=S)
+    Xg, X0, p = pipe_steps(w, precision, [7, 1, 42], n_tiles=n_tiles, t0=0.1)
+    Xo = oracle.step(X0[0], w.phase[0], 0.1, 0, 50, p)
+    assert np.abs(Xg[0] - Xo).max() <= tol * ELL
+
+
+@pytest.mark.parametrize("integrator", [ds.EULER, ds.HEUN])
+@pytest.mark.parametrize("tensor", [ds.OSEEN, ds.RPY])
+def test_pipeline_integrators_tensors_chunking_determinism(integrator, tensor):
+    """Euler and Heun, both tensors: the result does not depend on how the steps are split over launches and is bitwise
+    reproducible run to run (fixed summation trees, no atomics); host-buffer start equals device-buffer start."""
+    w = inputs.config5(B=1, S=300)
+    Xa, X0, p = pipe_steps(w, ds.F64, [101], n_tiles=20, tensor=tensor, integrator=integrator, t0=0.25)
+    Xb, _, _ = pipe_steps(w, ds.F64, [1, 33, 3, 64], n_tiles=20, tensor=tensor, integrator=integrator, t0=0.25)
+    Xc, _, _ = pipe_steps(w, ds.F64, [101], n_tiles=20, tensor=tensor, integrator=integrator, t0=0.25, host=True)
+    assert np.array_equal(Xa, Xb)
+    assert np.array_equal(Xa, Xc)
+    Xo = oracle.step(X0[0], w.phase[0], 0.25, 0, 101, p)
+    assert np.abs(Xa[0] - Xo).max() <= 1e-10 * ELL
+    # the one-pass kernel integrates the same equations (its sums are ordered differently: last bits only)
+    Xd, _, _ = pipe_steps(w, ds.F64, [101], n_tiles=20, tensor=tensor, integrator=integrator, t0=0.25, pipeline=0)
+    assert np.abs(Xa - Xd).max() <= 1e-11 * ELL
+
+
+@pytest.mark.parametrize("precision,tol", [(ds.F32, 1e-4), (ds.F64, 1e-10)])
+def test_pipeline_config4_headline_shape(precision, tol):
+    """C4 (N = 4096) in the launch configuration bench.py times: the library picks the pipelined kernel by itself (147
+    CTAs of 7 / 6 quads: halves of 4 + 3 and 3 + 3 quads); 200 steps against the oracle."""
+    w = inputs.config4()
+    s, p = make_system(w, precision)
+    with s:
+        assert s.pipeline_active()
+        X0 = rounded(w, precision)
+        s.set_state(dev(X0, precision), torch.as_tensor(w.phase, device="cuda"))
+        s.step(200)
+        out = torch.empty((1, w.N, 3), dtype=TDT[precision], device="cuda")
+        s.get_state(out)
+        V = torch.empty_like(out)
+        s.velocity(V)            # the one-pass kernel on the state the pipelined one left
+        torch.cuda.synchronize()
+    Xo = oracle.step(X0[0], w.phase[0], 0.0, 0, 200, p)
+    assert np.abs(out.cpu().numpy()[0].astype(np.float64) - Xo).max() <= tol * ELL
+    if precision == ds.F64:   # (in FP32 mode get_state rounds the FP64 state; the stiff spring amplifies that in V)
+        Vo = oracle.velocity(out.cpu().numpy()[0], w.phase[0], 200 * p.dt, p)
+        assert rel_l2(V.cpu().numpy()[0], Vo) <= 1e-9
+
+
+def test_pipeline_batch_and_noise():
+    """B = 5 systems of N = 600 in one launch (29 CTAs each) with k_B T > 0: per-system arrival counters, Philox
+    increments drawn by the service warp, steps split over calls."""
+    import dataclasses
+    w = inputs.config5(B=5, S=300)
+    Xg, X0, p = pipe_steps(w, ds.F64, [37, 63], n_tiles=29, kT=0.02, seed=0x1234567ABCDEF)
+    for b in range(w.B):
+        Xo = oracle.step(X0[b], w.phase[b], 0.0, 0, 100, dataclasses.replace(p, system=b))
+        assert np.abs(Xg[b] - Xo).max() <= 1e-9 * ELL
+
+
+# --------------------------------------------------------------------------------- variants no other test reaches
+@pytest.mark.parametrize("tensor", [ds.OSEEN, ds.RPY])
+@pytest.mark.parametrize("N", [8192, 16384])
+def test_apply_fp64_ring_mode(N, tensor):
+    """FP64 applies whose stream (48 B per sphere) exceeds shared memory: pack_user_kernel<double> + the TMA ring
+    (run_kernel<double, *, APPLY, false>), element by element."""
+    X, F = inputs.sweep_case(13 if N == 8192 else 14)
+    u = gpu_apply(X, F, ds.F64, tensor)
+    ref = oracle_apply(X, F, ds.F64, tensor)
+    assert rel_l2(u, ref) <= TOL[ds.F64]
+    assert np.abs(u - ref).max() <= 20 * TOL[ds.F64] * np.sqrt(np.mean(ref ** 2))
+
+
+@pytest.mark.parametrize("N", [8192, 8194])
+def test_apply_fp32_resident_ring_boundary(N):
+    """FP32 applies on both sides of the resident / ring boundary of the stream (N = 8192 is the last resident size)."""
+    X, F = inputs.apply_case(N, 81, 82)
+    u = gpu_apply(X, F, ds.F32, ds.RPY)
+    ref = oracle_apply(X, F, ds.F32, ds.RPY)
+    assert rel_l2(u, ref) <= TOL[ds.F32]
+    assert np.abs(u - ref).max() <= 20 * TOL[ds.F32] * np.sqrt(np.mean(ref ** 2))
+
+
+@pytest.mark.parametrize("integrator,n_steps", [(ds.HEUN, 2), (ds.EULER, 3)])
+def test_step_fp64_ring_mode(integrator, n_steps):
+    """N = 8192 in FP64: the stage input (384 KB) streams through the TMA ring with the blocking barrier
+    (run_kernel<double, *, VELOCITY / EULER / HEUN, false>)."""
+    w = inputs.config5(B=1, S=4096)
+    s, p = make_system(w, ds.F64, integrator=integrator)
+    X0 = rounded(w, ds.F64)
+    with s:
+        s.set_state(dev(X0, ds.F64), torch.as_tensor(w.phase, device="cuda"), t0=0.13)
+        out = torch.empty((1, w.N, 3), dtype=torch.float64, device="cuda")
+        V = torch.empty_like(out)
+        s.velocity(V)
+        s.step(n_steps)
+        s.get_state(out)
+        torch.cuda.synchronize()
+    assert rel_l2(V.cpu().numpy()[0], oracle.velocity(X0[0], w.phase[0], 0.13, p)) <= 1e-12
+    Xo = oracle.step(X0[0], w.phase[0], 0.13, 0, n_steps, p)
+    assert np.abs(out.cpu().numpy()[0] - Xo).max() <= 1e-10 * ELL
+
+
+def test_step_fp32_euler_ring_mode():
+    """N = 16384, FP32, Euler through the ring (run_kernel<float, *, EULER, false>)."""
+    w = inputs.config5(B=1, S=8192)
+    Xg, X0, p = gpu_steps(w, ds.F32, 3, integrator=ds.EULER)
+    Xo = oracle.step(X0[0], w.phase[0], 0.0, 0, 3, p)
+    assert np.abs(Xg[0] - Xo).max() <= 1e-4 * ELL
+
+
+def test_step_state_in_global_memory_odd_S_batch():
+    """The global-memory home of the per-row state with an odd number of dumbbells and two systems: the last quad of a
+    system has two rows, and the integrator must not touch the first spheres of the next system (S = 1051, 1 tile)."""
+    w = inputs.config5(B=2, S=1051)
+    s, p = make_system(w, ds.F64)
+    X0 = rounded(w, ds.F64)
+    with s:
+        s.set_tuning(1)
+        s.set_pipeline(0)
+        s.set_state(dev(X0, ds.F64), torch.as_tensor(w.phase, device="cuda"))
+        s.batch_step(6)
+        out = torch.empty((w.B, w.N, 3), dtype=torch.float64, device="cuda")
+        s.get_state(out)
+        torch.cuda.synchronize()
+    for b in range(w.B):
+        Xo = oracle.step(X0[b], w.phase[b], 0.0, 0, 6, p)
+        assert np.abs(out.cpu().numpy()[b] - Xo).max() <= 1e-10 * ELL
