@@ -1,13 +1,15 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the hot path of arXiv 1004.1932 on B200, beside the CPU oracle.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--sweep]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-sweep] [--quick]
 
 One bench "step" = one Heun time step of BASELINE.json config 4: a 3d random
 suspension of S = 2048 dumbbells (N = 4096 spheres), FP32 pair arithmetic, RPY tensor (the tensor
 the paper simulates with): force (Eq. 4) -> mobility apply (Eq. 3a,3b) -> predictor ->
 force -> mobility apply -> corrector, all on the device through ds_step (include/ds.h): one persistent
-kernel launch runs all K timed steps.
+kernel launch runs the K steps of a ds_step(K) call.  Timing: at least 50 ms of warm-up steps, then R back-to-back
+ds_step(K) launches (R such that the timed region exceeds 30 ms), each bracketed by CUDA events; ms_per_step is the
+median launch / K (min and max are in `timed_region`).
 Metric: ordered pair interactions per second, 2 N (N-1) per Heun step; timesteps/s is reported
 beside it for this and every other config.  The path does not shard: --gpus N runs N independent
 replicas, value = all replicas' pairs / the slowest replica's time.
@@ -30,8 +32,14 @@ if ROOT not in sys.path:
 
 METRIC = "pair_interactions_per_s"
 UNIT = "pairs/s"
-# Algorithmic FLOP per ordered pair (FMA = 2, rsqrt not counted), DESIGN.md "FLOP count":
-FLOP_PER_PAIR = {"oseen": 27, "rpy": 33}
+# Algorithmic FLOP per ordered pair (FMA = 2, rsqrt not counted): SURVEY.md 8(d)'s per-unit figure, the contract's count
+# (27 Oseen, 34 RPY).  The kernel's own pair body has 21 packed instructions for RPY, 12 of them FMA = 33 FLOP; the
+# fraction with that smaller count is reported beside it (roofline.frac_kernel_count).  DESIGN.md "FLOP count".
+FLOP_PER_PAIR = {"oseen": 27, "rpy": 34}
+FLOP_PER_PAIR_KERNEL = {"oseen": 27, "rpy": 33}
+# DRAM bytes (read + write) of one whole ds_step launch of the headline workload, from the ncu --set full capture of
+# the same command (profiles/r2_pipe_kernel_ncu_full.md): the path is ALU-bound and L2-resident
+NCU_DRAM_BYTES_PER_LAUNCH = {"f32": 321280, "f64": None}
 # ALU peaks derived in DESIGN.md "Roofline": SMs x lanes x 2 x f_SM(max).  FP32: 128 lanes/SM.  FP64: the
 # DFMA rate of B200 is what ds_peak_probe measures; the nominal figure used is 64 lanes/SM.
 N_SM, F32_LANES, F64_LANES = 148, 128, 64
@@ -45,7 +53,7 @@ def pairs_per_apply(N, B=1):
 class ClockSampler:
     """Samples SM clock, power and throttle reasons of one GPU through NVML while a timed region runs."""
 
-    def __init__(self, index, period=0.01):
+    def __init__(self, index, period=0.002):
         self.index, self.period = index, period
         self.sm, self.power, self.reasons = [], [], 0
         self.max_mhz = None
@@ -103,33 +111,55 @@ def _events(torch):
     return torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
 
 
-def time_steps(torch, ds, w, precision, tensor, n_steps, warmup, ranks=None, sampler=None):
-    """Device time of n_steps Heun steps of workload w through ds_step/ds_batch_step, state resident in
-    HBM.  Returns (seconds, launches in the timed region)."""
+WARM_S = 0.06      # at least this much device time of warm-up steps, whatever --warmup says (a lease may start at a low clock)
+TIMED_S = 0.03     # the timed region: back-to-back ds_step(K) launches until their device time exceeds this
+
+
+def time_steps(torch, ds, w, precision, tensor, n_steps, warmup, ranks=None, sampler=None, pipeline=None):
+    """Device time of n_steps Heun steps of workload w through ds_step/ds_batch_step, state resident in HBM.
+    Warm-up: `warmup` steps, repeated until WARM_S of device time has passed.  Timed: R back-to-back launches of
+    n_steps steps each (every launch bracketed by its own pair of CUDA events on the launching stream), R such that the
+    region exceeds TIMED_S; the reported time is the MEDIAN launch.  Returns (seconds per launch, launches per call,
+    info)."""
     npdt = np.float32 if precision == ds.F32 else np.float64
     stream = torch.cuda.current_stream()
     sc = w.scalars
     with ds.System(w.S, n_batch=w.B, precision=precision, tensor=tensor, integrator=ds.HEUN, a=sc["a"], eta=sc["eta"],
                    ell=sc["ell"], lam=sc["lam"], omega=sc["omega"], k0=sc["k0"], dt=sc["dt"],
                    device=torch.cuda.current_device(), stream=stream.cuda_stream) as s:
+        if pipeline is not None:
+            s.set_pipeline(pipeline)
         pos = torch.as_tensor(np.ascontiguousarray(w.pos, dtype=npdt), device="cuda")
         phase = torch.as_tensor(w.phase, device="cuda")
         s.set_state(pos, phase, 0.0)
         step = s.batch_step if w.B > 1 else s.step
-        step(max(int(warmup), 0))
-        torch.cuda.synchronize()
+        if sampler is not None:
+            sampler.__enter__()
+        # ---- warm-up ----
+        wsteps = max(int(warmup), 3)
         e0, e1 = _events(torch)
+        warm, wl = 0.0, 0
+        while warm < WARM_S and wl < 10000:
+            e0.record(stream)
+            step(wsteps)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            warm += e0.elapsed_time(e1) * 1e-3
+            wl += 1
+        est = warm / wl * (n_steps / wsteps)
+        reps = int(min(200, max(3, np.ceil(TIMED_S / max(est, 1e-9)))))
         if ranks is not None:
+            reps = int(ranks.max(reps))
             ranks.barrier()
         torch.cuda.synchronize()
         l0 = s.launch_count()
-        if sampler is not None:
-            sampler.__enter__()
-        e0.record(stream)
-        step(int(n_steps))
-        e1.record(stream)
+        ev = [_events(torch) for _ in range(reps)]
+        for a, b in ev:
+            a.record(stream)
+            step(int(n_steps))
+            b.record(stream)
         torch.cuda.synchronize()
-        launches = s.launch_count() - l0      # kernels launched inside the timed region
+        launches = (s.launch_count() - l0) // reps      # kernels launched per timed ds_step call
         if sampler is not None:
             sampler.__exit__()
         if ranks is not None:
@@ -139,7 +169,11 @@ def time_steps(torch, ds, w, precision, tensor, n_steps, warmup, ranks=None, sam
         torch.cuda.synchronize()
         if not bool(torch.isfinite(out).all()):
             raise RuntimeError("non-finite state after the timed steps")
-        return e0.elapsed_time(e1) * 1e-3, launches
+        t = np.array([a.elapsed_time(b) * 1e-3 for a, b in ev])
+        info = {"repeats": reps, "warmup_launches": wl, "warmup_device_ms": warm * 1e3,
+                "ms_per_step_min": 1e3 * t.min() / n_steps, "ms_per_step_max": 1e3 * t.max() / n_steps,
+                "timed_region_ms": 1e3 * t.sum(), "pipelined_kernel": bool(s.pipeline_active())}
+        return float(np.median(t)), int(launches), info
 
 
 def time_steps_cold_l2(torch, ds, w, precision, tensor, n_steps):
@@ -348,9 +382,36 @@ def avg_model_extra(torch, ds, sizes=(729, 2048, 8192)):
     return avg
 
 
+def cpu_apply_sweep(inputs):
+    """the oracle's mobility apply (RPY, FP64) timed single-threaded and on all host cores at every sweep
+    size up to N = 16384, and once at N = 65536 on all cores.  Pair-interactions/s, pairs = N (N - 1)."""
+    import oracle
+    cores = oracle.max_threads()
+    out = {"cores": cores, "kind": "oracle", "tensor": "rpy", "unit": UNIT}
+    for lg in range(8, 15):
+        Xs, Fs = inputs.sweep_case(lg)
+        n = 1 << lg
+        row = {}
+        for name, th in (("single_thread", 1), ("all_cores", cores)):
+            oracle.set_threads(th)
+            reps = max(1, min(20, int(2e8 * th / (n * n))))
+            t0 = time.perf_counter()
+            for _ in range(reps):
+                oracle.mobility_apply(Xs, Fs, 1.0, 1.0, oracle.RPY)
+            row[name] = pairs_per_apply(n) * reps / (time.perf_counter() - t0)
+        out[f"N{n}"] = row
+    Xs, Fs = inputs.sweep_case(16)
+    oracle.set_threads(cores)
+    t0 = time.perf_counter()
+    oracle.mobility_apply(Xs, Fs, 1.0, 1.0, oracle.RPY)
+    out["N65536"] = {"all_cores": pairs_per_apply(65536) / (time.perf_counter() - t0)}
+    return out
+
+
 def extras(torch, ds, inputs, w, args, precision, tensor):
     """Beside the headline: the standalone apply at N = 4096 (4 variants), timesteps/s of every config,
-    the cold-L2 per-step figure, and (with --sweep) the N = 256 .. 65536 apply sweep."""
+    the cold-L2 per-step figure, the N = 256 .. 65536 apply sweep (BASELINE.json configs[4]) and the oracle's apply
+    timings at the sweep sizes; --no-sweep leaves the last two out."""
     extra = {}
     # apply at N = 4096, all four variants (the standalone sweep of config 4)
     Xa, Fa = inputs.apply_case(4096, 1004, 2004)
@@ -368,19 +429,21 @@ def extras(torch, ds, inputs, w, args, precision, tensor):
     for name, mk, pr, nst in (("C1_N16_f64", inputs.config1, ds.F64, 10_000),
                               ("C2_N128_f32", inputs.config2, ds.F32, 10_000),
                               ("C2_N128_f64", inputs.config2, ds.F64, 10_000),
-                              ("C3_N1024_f32", inputs.config3, ds.F32, 10_000),
+                              ("C3_N1024_f32", inputs.config3, ds.F32, 100_000),
                               ("C4_N4096_f32", inputs.config4, ds.F32, 1000),
                               ("C4_N4096_f64", inputs.config4, ds.F64, 1000),
-                              ("C5_B64_N512_f32", inputs.config5, ds.F32, 2000)):
+                              ("C5_B64_N512_f32", inputs.config5, ds.F32, 10_000)):
         wc = w if mk is inputs.config4 else mk()
-        t, _ = time_steps(torch, ds, wc, pr, ds.RPY, nst, 64)
+        t, _, info = time_steps(torch, ds, wc, pr, ds.RPY, nst, 64)
         cfgs[name] = {"timesteps_per_s": nst / t, "pairs_per_s": nst * 2 * pairs_per_apply(wc.N, wc.B) / t,
-                      "steps_timed": nst}
+                      "us_per_stage": 1e6 * t / (2 * nst), "steps_per_launch": nst, "repeats": info["repeats"],
+                      "pipelined_kernel": info["pipelined_kernel"]}
     extra["configs_rpy_heun"] = cfgs
     extra["avg_model_eq9"] = avg_model_extra(torch, ds)
     extra["cold_l2"] = {"ms_per_step": 1e3 * time_steps_cold_l2(torch, ds, w, precision, tensor, 30),
                         "steps": 30, "flush": "512 MiB fill before every step"}
-    if args.sweep:
+    if not args.no_sweep:
+        # BASELINE.json configs[4]: scaling sweep of one mobility apply, N = 256 .. 65536, FP32, both tensors
         sw = {}
         for lg in range(8, 17):
             Xs, Fs = inputs.sweep_case(lg)
@@ -392,6 +455,7 @@ def extras(torch, ds, inputs, w, args, precision, tensor):
                                        "frac_of_alu_peak": pairs_per_apply(n) * FLOP_PER_PAIR[tname] / t /
                                        (N_SM * F32_LANES * 2 * 1.965e9)}
         extra["sweep_f32"] = sw
+        extra["cpu_apply"] = cpu_apply_sweep(inputs)
     return extra
 
 
@@ -410,9 +474,9 @@ def run_ours(args, ranks):
     N = w.N
     flop_pair = FLOP_PER_PAIR[args.tensor]
 
-    # ---- the timed region: K Heun steps, state resident in HBM ----
+    # ---- the timed region: K Heun steps per launch, state resident in HBM; R launches, median (time_steps) ----
     sampler = ClockSampler(torch.cuda.current_device())
-    sec, launches = time_steps(torch, ds, w, precision, tensor, args.steps, max(args.warmup, 3), ranks, sampler)
+    sec, launches, tinfo = time_steps(torch, ds, w, precision, tensor, args.steps, max(args.warmup, 3), ranks, sampler)
     clocks = sampler.summary()
     sec_max = ranks.max(sec)
     pairs_step = 2 * pairs_per_apply(N)
@@ -422,30 +486,48 @@ def run_ours(args, ranks):
     e_sec, h2d, d2h, e_launches = time_e2e(torch, ds, w, precision, tensor, args.steps, args.warmup, ranks)
     e_value = ranks.sum(args.steps * pairs_step) / ranks.max(e_sec)
 
-    line = None
-    if ranks.rank == 0:
-        kernel_s = sec / (2 * args.steps)          # the one persistent launch runs 2 mobility stages per Heun step
-        lanes = F32_LANES if args.precision == "f32" else F64_LANES
+    def roofline_of(prec_name, sec_launch, info):
+        """roofline object of one ds_step(K) launch: 2 K mobility stages of N (N - 1) ordered pairs each."""
+        kernel_s = sec_launch / (2 * args.steps)
+        lanes = F32_LANES if prec_name == "f32" else F64_LANES
         peak_nominal = N_SM * lanes * 2 * 1.965e9 * 1e-12
         achieved = pairs_per_apply(N) * flop_pair / kernel_s * 1e-12
         roof = {"bound": "alu", "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s",
-                "frac": achieved / peak_nominal, "traffic": None,
-                "traffic_note": "ALU-bound path: DRAM bytes of the whole 50-step launch by ncu --set full are 0.37 MB "
-                                "(profiles/r1g_run_kernel_ncu_full.md); the algorithmic traffic is the 96 KB L2-resident "
-                                "stream read by each CTA per stage",
-                "kernel": "ds::run_kernel<float|double, tensor> (persistent: per stage pair sum + split-beta reduce + "
-                          "Eq. (3a) + Heun update + Eq. (4) + inter-CTA barrier; ONE launch for all timed steps)",
-                "stage_us": kernel_s * 1e6, "stages_per_step": 2, "launch_us": sec * 1e6,
+                "frac": achieved / peak_nominal,
+                "frac_kernel_count": achieved / peak_nominal * FLOP_PER_PAIR_KERNEL[args.tensor] / flop_pair,
+                "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(prec_name),
+                "traffic_note": "DRAM bytes (read + write) of one 50-step launch by ncu --set full "
+                                "(profiles/r2_pipe_kernel_ncu_full.md); the algorithmic traffic of the ALU-bound path is the "
+                                "L2-resident stream (24 B per sphere and stage in FP32) read by each CTA once per stage",
+                "kernel": ("ds::pipe_kernel" if info["pipelined_kernel"] else "ds::run_kernel") +
+                          "<float|double, tensor, Heun> (persistent: per stage pair sums + reduction + Eq. (3a) + Heun update + "
+                          "Eq. (4) + stage hand-over; ONE launch for all K steps of a ds_step call)",
+                "stage_us": kernel_s * 1e6, "stages_per_step": 2, "launch_us": sec_launch * 1e6,
                 "flop_per_launch": args.steps * 2 * pairs_per_apply(N) * flop_pair,
-                "peak_kind": f"derived: {N_SM} SMs x {lanes} {args.precision} FMA lanes x 2 x 1.965 GHz "
+                "peak_kind": f"derived: {N_SM} SMs x {lanes} {prec_name} FMA lanes x 2 x 1.965 GHz "
                              f"(MEASURED_PEAKS.json sm_max_mhz); MEASURED_PEAKS.json has no ALU entry",
-                "flop_per_pair": flop_pair, "pairs_per_stage": pairs_per_apply(N)}
+                "flop_per_pair": flop_pair, "flop_per_pair_kernel": FLOP_PER_PAIR_KERNEL[args.tensor],
+                "pairs_per_stage": pairs_per_apply(N), "timing": info}
+        return roof
+
+    line = None
+    if ranks.rank == 0:
+        roof = roofline_of(args.precision, sec, tinfo)
         if clocks.get("sm_mhz"):
-            roof["frac_at_sampled_clock"] = achieved / (N_SM * lanes * 2 * clocks["sm_mhz"] * 1e6 * 1e-12)
+            lanes = F32_LANES if args.precision == "f32" else F64_LANES
+            roof["frac_at_sampled_clock"] = roof["achieved"] / (N_SM * lanes * 2 * clocks["sm_mhz"] * 1e6 * 1e-12)
         probe = peak_probe(ds, torch)
         if probe:
             roof["measured_fma_chain"] = probe
-            roof["frac_of_measured_chain"] = achieved / probe[args.precision + "_tflops"]
+            roof["frac_of_measured_chain"] = roof["achieved"] / probe[args.precision + "_tflops"]
+        # the paper's own arithmetic is FP64 (PAPER.md:232): the same workload and launch in the other precision
+        other = "f64" if args.precision == "f32" else "f32"
+        o_sec, _, o_info = time_steps(torch, ds, w, ds.F64 if other == "f64" else ds.F32, tensor, args.steps,
+                                      max(args.warmup, 3))
+        roof_other = roofline_of(other, o_sec, o_info)
+        roof_other["timesteps_per_s"] = args.steps / o_sec
+        if probe:
+            roof_other["frac_of_measured_chain"] = roof_other["achieved"] / probe[other + "_tflops"]
 
         extra = None if args.quick else extras(torch, ds, inputs, w, args, precision, tensor)
 
@@ -470,8 +552,11 @@ def run_ours(args, ranks):
                 "e2e": {"value": e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                         "ms_per_step": 1e3 * e_sec / args.steps,
                         "path": "ds_set_state(host pos, host phase) + ds_step(1) + ds_get_state(host pos), pinned"},
-                "gpu_launches": int(launches),
-                "roofline": roof, "cpu_baseline": cpu, "extra": extra}
+                "gpu_launches": int(launches * tinfo["repeats"]),
+                "timed_region": {"launches": tinfo["repeats"], "steps_per_launch": args.steps, "statistic": "median launch",
+                                 "ms_per_step_min": tinfo["ms_per_step_min"], "ms_per_step_max": tinfo["ms_per_step_max"],
+                                 "warmup_device_ms": tinfo["warmup_device_ms"]},
+                "roofline": roof, "roofline_" + other: roof_other, "cpu_baseline": cpu, "extra": extra}
     ranks.barrier()
     if line is not None:
         print(json.dumps(line), flush=True)
@@ -486,7 +571,7 @@ def main():
     ap.add_argument("--precision", choices=["f32", "f64"], default="f32")
     ap.add_argument("--tensor", choices=["oseen", "rpy"], default="rpy")
     ap.add_argument("--cpu-steps", type=int, default=20, help="oracle Heun steps timed for cpu_baseline")
-    ap.add_argument("--sweep", action="store_true", help="add the N = 256 .. 65536 apply sweep to extra")
+    ap.add_argument("--no-sweep", action="store_true", help="leave the N = 256 .. 65536 apply sweep and the oracle's apply timings out of extra")
     ap.add_argument("--quick", action="store_true", help="headline + e2e only (used under ncu)")
     ap.add_argument("--avg-model", action="store_true",
                     help="only the averaged-model timing of extra.avg_model_eq9 at S = 729 (used under ncu)")

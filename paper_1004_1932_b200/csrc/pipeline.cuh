@@ -147,48 +147,30 @@ __global__ void __launch_bounds__(PIPE_NT, 1) pipe_kernel(const PipeArgs A) {
             mbar_init(mb_xi + h, 1);
         }
         mbar_fence_init();
-        // Which warp does what in the two passes (stage-invariant).  The 16 warps of a pass are dealt to its nqp quads, m = 16 / nqp
-        // or one more each; place (quad, sub), sub < m, walks the units 32 sub + lane + k * 32 m of a region.  Places go to
-        // the four SM sub-partitions (warp % 4) so that their iteration counts balance over the whole stage; sub-partition
-        // 0, which also hosts the service warp, gets a little less.
-        int load[4] = {2, 0, 0, 0};
-        for (int h = 0; h < 2; ++h) {
-            const int nqp = h == 0 ? nqA : nq - nqA, rows_h = h == 0 ? rowsA : rowsB;
-            const int own0 = h == 0 ? ownA : ownB, own1 = own0 + rows_h / W;
-            int used[4] = {0, 0, 0, 0};
-            for (int w = 0; w < PIPE_CW; ++w) ptab[(h * PIPE_CW + w) * 3] = make_int4(0, 0, 0, 0);
-            if (nqp == 0) continue;
-            const int mb = PIPE_CW / nqp, mr = PIPE_CW % nqp;          // quad q gets mb + (q < mr) warps
-            for (int sub = 0; sub <= mb; ++sub) {                      // heavier places (small sub) first
-                for (int quad = 0; quad < nqp; ++quad) {
-                    const int m = mb + (quad < mr ? 1 : 0), n_jg = 32 * m;
-                    if (sub >= m) continue;
-                    int4 q[2];
-                    int tot = 0;
-                    for (int reg = 0; reg < 2; ++reg) {
-                        const int Ur = A.reg_units[reg];
-                        const int its = (Ur + n_jg - 1) / n_jg;
-                        // the last iteration is skipped by warps whose 32 units all lie behind the region
-                        const int its_w = its - ((its > 0 && (its - 1) * n_jg + 32 * sub >= Ur) ? 1 : 0);
-                        int g_lo = its_w, g_hi = its_w;     // iterations that may hold own units (alpha == beta): region h only
-                        if (reg == h && rows_h > 0) {
-                            g_lo = own0 / n_jg; g_hi = (own1 - 1) / n_jg + 1;
-                            g_lo = g_lo < its_w ? g_lo : its_w; g_hi = g_hi < its_w ? g_hi : its_w;
-                        }
-                        q[reg] = make_int4(its_w, g_lo, g_hi, 0);
-                        tot += its_w;
-                    }
-                    int best = -1;
-                    for (int sp = 3; sp >= 0; --sp)
-                        if (used[sp] < 4 && (best < 0 || load[sp] < load[best])) best = sp;
-                    const int w = best + 4 * used[best];
-                    used[best] += 1; load[best] += tot;
-                    int4 *e = ptab + (h * PIPE_CW + w) * 3;
-                    q[0].w = quad * mb + (quad < mr ? quad : mr) + sub;   // slot of this place's sums in scr
-                    e[0] = make_int4(1, quad, sub, m); e[1] = q[0]; e[2] = q[1];
-                }
+    }
+    // Which warp does what in the two passes (stage-invariant).  The 16 warps of a pass are dealt to its nqp quads, m = 16 / nqp
+    // or one more each; place (quad, sub), sub < m, walks the units 32 sub + lane + k * 32 m of a region.
+    // Step 1, one thread per (pass, m class, sub, region): the place's loop bounds (scr is free until the first pass ends).
+    int4 *const bounds = reinterpret_cast<int4 *>(scr);               // [2 passes][2 classes][16 subs][2 regions]
+    if (tid >= 64 && tid < 192) {
+        const int i = tid - 64, h = i >> 6, cls = (i >> 5) & 1, sub = (i >> 1) & 15, reg = i & 1;
+        const int nqp = h == 0 ? nqA : nq - nqA, rows_h = h == 0 ? rowsA : rowsB;
+        const int own0 = h == 0 ? ownA : ownB, own1 = own0 + rows_h / W;
+        int4 q = make_int4(0, 0, 0, 0);
+        if (nqp > 0) {
+            const int m = PIPE_CW / nqp + cls, n_jg = 32 * m;
+            const int Ur = A.reg_units[reg];
+            const int its = (Ur + n_jg - 1) / n_jg;
+            // the last iteration is skipped by warps whose 32 units all lie behind the region
+            const int its_w = its - ((its > 0 && (its - 1) * n_jg + 32 * sub >= Ur) ? 1 : 0);
+            int g_lo = its_w, g_hi = its_w;     // iterations that may hold own units (alpha == beta): region h only
+            if (reg == h && rows_h > 0) {
+                g_lo = own0 / n_jg; g_hi = (own1 - 1) / n_jg + 1;
+                g_lo = g_lo < its_w ? g_lo : its_w; g_hi = g_hi < its_w ? g_hi : its_w;
             }
+            q = make_int4(its_w, g_lo, g_hi, 0);
         }
+        bounds[i] = q;
     }
     // far-away zero-force pad units behind each region (never overwritten: the bulk copies bring the real units only)
     for (int h = 0; h < 2; ++h) {
@@ -196,6 +178,39 @@ __global__ void __launch_bounds__(PIPE_NT, 1) pipe_kernel(const PipeArgs A) {
         for (int j = 3 * A.reg_units[h] + tid; j < 3 * A.buf_units[h]; j += PIPE_NT) bp[j] = pad_piece<T>(j % 3);
     }
     __syncthreads();
+    if (tid == 0) {
+        // Step 2: places go to the four SM sub-partitions (warp % 4) so that their iteration counts balance over the whole
+        // stage; sub-partition 0, which also hosts the service warp, gets a little less.
+        int load0 = 2, load1 = 0, load2 = 0, load3 = 0;
+        for (int h = 0; h < 2; ++h) {
+            const int nqp = h == 0 ? nqA : nq - nqA;
+            int used0 = 0, used1 = 0, used2 = 0, used3 = 0;
+            for (int w = 0; w < PIPE_CW; ++w) ptab[(h * PIPE_CW + w) * 3] = make_int4(0, 0, 0, 0);
+            if (nqp == 0) continue;
+            const int mb = PIPE_CW / nqp, mr = PIPE_CW % nqp;          // quad q gets mb + (q < mr) warps
+            for (int sub = 0; sub <= mb; ++sub) {                      // heavier places (small sub) first
+                for (int quad = 0; quad < nqp; ++quad) {
+                    const int cls = quad < mr ? 1 : 0, m = mb + cls;
+                    if (sub >= m) continue;
+                    int4 qa = bounds[((h * 2 + cls) * 16 + sub) * 2], qb = bounds[((h * 2 + cls) * 16 + sub) * 2 + 1];
+                    const int tot = qa.x + qb.x;
+                    int best = -1, bl = 0;
+                    if (used3 < 4) { best = 3; bl = load3; }
+                    if (used2 < 4 && (best < 0 || load2 < bl)) { best = 2; bl = load2; }
+                    if (used1 < 4 && (best < 0 || load1 < bl)) { best = 1; bl = load1; }
+                    if (used0 < 4 && (best < 0 || load0 < bl)) { best = 0; bl = load0; }
+                    int u;
+                    if (best == 3) { u = used3++; load3 += tot; }
+                    else if (best == 2) { u = used2++; load2 += tot; }
+                    else if (best == 1) { u = used1++; load1 += tot; }
+                    else { u = used0++; load0 += tot; }
+                    int4 *e = ptab + (h * PIPE_CW + best + 4 * u) * 3;
+                    qa.w = quad * mb + (quad < mr ? quad : mr) + sub;   // slot of this place's sums in scr
+                    e[0] = make_int4(1, quad, sub, m); e[1] = qa; e[2] = qb;
+                }
+            }
+        }
+    }
     {
         const double tn = time_of_step(A.t0, A.n0, A.dt);
         T *s0 = stream_of(0);
@@ -294,16 +309,13 @@ __global__ void __launch_bounds__(PIPE_NT, 1) pipe_kernel(const PipeArgs A) {
     } else {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(PIPE_REGS_SERVICE));   // all four warps of the service warpgroup
     }
-    if (warp == PIPE_CW) {
-        // =========================== service warp ===========================
-        // stream 0 is complete once every CTA has arrived once per region
-        if (lane == 0) {
-            red_release_gpu(cnt + 0, 1ULL);
-            red_release_gpu(cnt + 1, 1ULL);
-            mbar_arrive(mb_xi + 0);
-            mbar_arrive(mb_xi + 1);
-        }
-        auto fetch_region = [&](int h, int g) {   // lane 0: region h of stream g -> shared memory, once every CTA has published it
+    if (warp >= PIPE_CW) {
+        // =========================== service warpgroup ===========================
+        // All four warps share the per-element work of a half's tail (one state element per thread); warp 16, the lead,
+        // also evaluates Eq. (4), publishes, signals and prefetches.  They meet at named barrier 1.
+        const int st_id = tid - 32 * PIPE_CW;      // 0 .. 127
+        const bool lead = warp == PIPE_CW;
+        auto fetch_region = [&](int h, int g) {   // one thread: region h of stream g -> shared memory, once every CTA has published it
             const unsigned long long target = A.cnt_base + (unsigned long long)(g + 1) * (unsigned long long)A.n_cta;
             while (ld_acquire_gpu(cnt + h) < target) {}
             fence_proxy_async();
@@ -316,28 +328,39 @@ __global__ void __launch_bounds__(PIPE_NT, 1) pipe_kernel(const PipeArgs A) {
                 mbar_arrive(mb_full + h);
             }
         };
-        if (lane == 0 && n_stage > 0) { fetch_region(0, 0); fetch_region(1, 0); }
+        if (lead && lane == 0) {
+            // stream 0 is complete once every CTA has arrived once per region
+            red_release_gpu(cnt + 0, 1ULL);
+            red_release_gpu(cnt + 1, 1ULL);
+            mbar_arrive(mb_xi + 0);
+            mbar_arrive(mb_xi + 1);
+            if (n_stage > 0) { fetch_region(0, 0); fetch_region(1, 0); }
+        }
         __syncwarp();
         for (int g = 0; g < n_stage; ++g) {
             const uint32_t par = (uint32_t)g & 1u;
             const bool pred = HEUN && (g & 1) == 0, corr = HEUN && (g & 1) == 1;
             const long long nstep = A.n0 + (HEUN ? (g >> 1) : g);
-            if (!HEUN || (g & 1) == 0) {   // stroke length at the end of this step, L(t_{n+1}), once per step
+            if (lead && (!HEUN || (g & 1) == 0)) {   // stroke length at the end of this step, L(t_{n+1}), once per step
                 const double t1 = time_of_step(A.t0, nstep + 1, A.dt);
                 for (int sl = lane; sl < nd; sl += 32) Ls[sl] = stroke_length(t1, phs[sl], A.ell, A.lambda, A.omega);
             }
             const bool last = g + 1 == n_stage;
             T *const snext = stream_of(g + 1);
+            const double cdt = corr ? 0.5 * A.dt : A.dt;
 #pragma unroll 1
             for (int h = 0; h < 2; ++h) {
                 const int nqp = h == 0 ? nqA : nq - nqA, rows_h = h == 0 ? rowsA : rowsB, rbase = h == 0 ? 0 : rowsA;
                 const int mb = nqp > 0 ? PIPE_CW / nqp : 0, mr = nqp > 0 ? PIPE_CW % nqp : 0;
+                // the thread's first element: everything that does not depend on the pass's sums is fetched before the wait
+                const bool has0 = st_id < 3 * rows_h;
+                const int E0 = 3 * rbase + st_id;
+                const double f0 = has0 ? Fs[E0] : 0.0, x0s = has0 ? Xs[E0] : 0.0, v10 = (has0 && corr) ? V1s[E0] : 0.0;
                 mbar_wait(mb_part + h, par);
                 PIPE_PROBE(16 + 6 * h);
-                // Eq. (3a), the 1/(8 pi mu) factor and the integrator in FP64, one state element per lane
-                const double cdt = corr ? 0.5 * A.dt : A.dt;
+                // Eq. (3a), the 1/(8 pi mu) factor and the integrator in FP64, one state element per thread
 #pragma unroll 1
-                for (int e = lane; e < 3 * rows_h; e += 32) {
+                for (int e = st_id; e < 3 * rows_h; e += 128) {
                     const int rl = e / 3, cc = e - 3 * rl, quad = rl >> 2, k = rl & 3;
                     const int m = mb + (quad < mr ? 1 : 0);
                     const T *sp = scr + (h * PIPE_CW + quad * mb + (quad < mr ? quad : mr)) * 12 + 3 * k + cc;
@@ -346,43 +369,46 @@ __global__ void __launch_bounds__(PIPE_NT, 1) pipe_kernel(const PipeArgs A) {
                     for (int j = 0; j < m; ++j) sacc += sp[12 * j];
                     const double sum = (double)sacc;
                     const int E = 3 * rbase + e;
-                    const double v = A.self_mob * Fs[E] + A.pre * sum;
-                    const double w = corr ? V1s[E] + v : v;
-                    double xn = Xs[E] + cdt * w;
+                    const bool first = e == st_id;
+                    const double v = A.self_mob * (first ? f0 : Fs[E]) + A.pre * sum;
+                    const double w = corr ? (first ? v10 : V1s[E]) + v : v;
+                    double xn = (first ? x0s : Xs[E]) + cdt * w;
                     if (A.noise_amp != 0.0) xn += A.noise_amp * noise_normal(A.seed, nstep, b, 3 * r0 + E);
                     if (pred) V1s[E] = v; else Xs[E] = xn;
                     Xc[E] = xn;
                     XcT[E] = (T)xn;
                 }
-                __syncwarp();
+                asm volatile("bar.sync 1, 128;" ::: "memory");
                 PIPE_PROBE(28 + h);
-                // Eq. (4) at the new positions and time; publish the half's rows of the next stage's stream
-                for (int sl = lane; sl < (rows_h >> 1); sl += 32) {
-                    const int row = rbase + 2 * sl;
-                    double x0[3], x1[3], F0[3];
+                if (lead) {
+                    // Eq. (4) at the new positions and time; publish the half's rows of the next stage's stream
+                    for (int sl = lane; sl < (rows_h >> 1); sl += 32) {
+                        const int row = rbase + 2 * sl;
+                        double x0[3], x1[3], F0[3];
 #pragma unroll
-                    for (int cc = 0; cc < 3; ++cc) { x0[cc] = Xc[3 * row + cc]; x1[cc] = Xc[3 * row + 3 + cc]; }
-                    dumbbell_force(x0, x1, Ls[row >> 1], A.k0, F0);
+                        for (int cc = 0; cc < 3; ++cc) { x0[cc] = Xc[3 * row + cc]; x1[cc] = Xc[3 * row + 3 + cc]; }
+                        dumbbell_force(x0, x1, Ls[row >> 1], A.k0, F0);
 #pragma unroll
-                    for (int cc = 0; cc < 3; ++cc) { Fs[3 * row + cc] = F0[cc]; Fs[3 * row + 3 + cc] = -F0[cc]; }
-                    if (!last) publish_dumbbell(own_units(snext, h), nullptr, 0u, 2 * sl, x0, x1, F0);
-                }
-                PIPE_PROBE(30 + h);
-                if (!last) fence_proxy_async_global();
-                __syncwarp();
-                PIPE_PROBE(17 + 6 * h);
-                if (lane == 0) {
-                    if (!last) red_release_gpu(cnt + h, 1ULL);   // this CTA's half of stream g + 1 is out
-                    PIPE_PROBE(20 + 6 * h);
-                    mbar_arrive(mb_xi + h);                      // ... and its rows of stage g + 1 are in XcT
-                    if (!last) {
-                        mbar_wait(mb_empty + h, par);            // every compute warp is past the region's old content
-                        PIPE_PROBE(18 + 6 * h);
-                        fetch_region(h, g + 1);
-                        PIPE_PROBE(19 + 6 * h);
+                        for (int cc = 0; cc < 3; ++cc) { Fs[3 * row + cc] = F0[cc]; Fs[3 * row + 3 + cc] = -F0[cc]; }
+                        if (!last) publish_dumbbell(own_units(snext, h), nullptr, 0u, 2 * sl, x0, x1, F0);
                     }
+                    PIPE_PROBE(30 + h);
+                    if (!last) fence_proxy_async_global();
+                    __syncwarp();
+                    PIPE_PROBE(17 + 6 * h);
+                    if (lane == 0) {
+                        if (!last) red_release_gpu(cnt + h, 1ULL);   // this CTA's half of stream g + 1 is out
+                        PIPE_PROBE(20 + 6 * h);
+                        mbar_arrive(mb_xi + h);                      // ... and its rows of stage g + 1 are in XcT
+                        if (!last) {
+                            mbar_wait(mb_empty + h, par);            // every compute warp is past the region's old content
+                            PIPE_PROBE(18 + 6 * h);
+                            fetch_region(h, g + 1);
+                            PIPE_PROBE(19 + 6 * h);
+                        }
+                    }
+                    __syncwarp();
                 }
-                __syncwarp();
             }
         }
     }
