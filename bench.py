@@ -376,9 +376,10 @@ def avg_model_extra(torch, ds, sizes=(729, 2048, 8192)):
                          # 93 FLOP per ordered dumbbell pair of Eq. (9c,d) as the kernel evaluates it (FMA = 2)
                          "flop_per_pair": AVG_FLOP_PER_PAIR,
                          "frac_of_alu_peak_stepping": 2 * S_ * (S_ - 1) * AVG_FLOP_PER_PAIR / ts / (N_SM * F32_LANES * 2 * 1.965e9),
-                         "note": "ds_avg_rhs on device buffers (sin/cos table kernel + pair kernel per call) and ds_avg_step "
-                                 "(2 launches per Heun step, FP64 state); FP32 pair arithmetic, 32 dumbbells x 8 slices per "
-                                 "CTA, clusters of <= 8 CTAs per block of dumbbells"}
+                         "note": "ds_avg_rhs on device buffers (sin/cos table kernel + pair kernel per call: 32 dumbbells x 8 "
+                                 "slices per CTA, clusters of <= 8 CTAs per block of dumbbells) and ds_avg_step (S <= 4096: one "
+                                 "device-resident cooperative launch for all steps, tagged hand-over between stages; larger S: 2 "
+                                 "launches per Heun step); FP64 state, FP32 pair arithmetic"}
     return avg
 
 

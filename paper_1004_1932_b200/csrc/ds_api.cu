@@ -110,6 +110,9 @@ struct ds_system {
     Buf ap_units, st_a, st_b, st_c;
     Buf avg;                                    // FP64 scratch of the stroke-averaged model (Eq. 9)
     Buf avg_sc;                                 // its sin/cos table
+    Buf avg_xch;                                // tagged exchange buffers of the device-resident stepping (averaged.cuh)
+    unsigned int avg_tag = 1;                   // next unused tag (0 = never written)
+    size_t avg_xch_records = 0;
 };
 
 namespace {
@@ -549,6 +552,55 @@ int launch_avg_rhs(ds_system *s, const IO *R, const IO *N, int S, IO *dR, IO *dN
     return launch_avg_rhs_t<float, IO>(s, R, N, S, dR, dN, U);
 }
 
+// Device-resident Heun stepping of Eq. (9) (averaged.cuh, avg_persist_kernel) when the whole input of a stage fits one
+// CTA's shared memory and the grid is co-resident; *used tells the caller whether it ran.
+constexpr int AVG_PERSIST_MAX_S = 4096;
+template <typename T>
+int avg_step_persistent_t(ds_system *s, double *Rd, double *Nd, int S, double dt, long long n_steps, bool *used) {
+    *used = false;
+    if (S > AVG_PERSIST_MAX_S || n_steps < 1) return DS_OK;
+    constexpr int W = ds::Pack<T>::W, PPR = 8 * (int)sizeof(T) / 8;
+    int G = S < s->num_sms ? S : s->num_sms;
+    const int ns = (S + G - 1) / G;
+    G = (S + ns - 1) / ns;
+    if (ns > 64) return DS_OK;
+    const int nu = (S + W - 1) / W, n_sl = ds::AVG_NT / ns, n_out = 6 * ns;
+    const size_t smem = (size_t)nu * 64 + (size_t)n_sl * n_out * sizeof(T) + (size_t)n_out * sizeof(double) + (size_t)ns * 20 * sizeof(double);
+    if (smem > (size_t)ds::SMEM_MAX) return DS_OK;
+    const size_t rec_bytes = (size_t)PPR * 16, need = 2 * (size_t)S * rec_bytes;
+    const long long n_stage = 2 * n_steps;
+    if (s->avg_xch.cap < need || (unsigned long long)s->avg_tag + (unsigned long long)n_stage + 2ULL >= 0xffffffffULL) {
+        DS_TRY(ensure(s->avg_xch, need));
+        CU_TRY(cudaMemsetAsync(s->avg_xch.p, 0, s->avg_xch.cap, s->stream));   // tag 0 = never written
+        s->avg_tag = 1;
+    }
+    auto kern = ds::avg_persist_kernel<T>;
+    static SmemOptIn opt_in;
+    DS_TRY(opt_in.ensure((const void *)kern, s->P.device));
+    long long left = n_steps;
+    while (left > 0) {
+        const long long k = left < MAX_STEPS_PER_LAUNCH ? left : MAX_STEPS_PER_LAUNCH;
+        ds::AvgPersistArgs A;
+        memset(&A, 0, sizeof A);
+        A.S = S; A.ns = ns; A.R = Rd; A.N = Nd; A.sc = (const double2 *)s->avg_sc.p; A.C = avg_consts(s); A.dt = dt; A.n_steps = k;
+        A.xch[0] = (uint4 *)s->avg_xch.p; A.xch[1] = (uint4 *)((char *)s->avg_xch.p + (size_t)S * rec_bytes);
+        A.tag0 = s->avg_tag;
+        A.probe = s->probe;
+        void *args[] = {(void *)&A};
+        CU_TRY(cudaLaunchCooperativeKernel((const void *)kern, dim3((unsigned)G), dim3(ds::AVG_NT), args, smem, s->stream));
+        s->launches += 1;
+        s->avg_tag += (unsigned int)(2 * k) + 1u;
+        left -= k;
+    }
+    *used = true;
+    return DS_OK;
+}
+
+int avg_step_persistent(ds_system *s, double *Rd, double *Nd, int S, double dt, long long n_steps, bool *used) {
+    if (s->P.precision == DS_F64) return avg_step_persistent_t<double>(s, Rd, Nd, S, dt, n_steps, used);
+    return avg_step_persistent_t<float>(s, Rd, Nd, S, dt, n_steps, used);
+}
+
 // user buffer (device or host, user precision, n elements) -> FP64 device array dst
 int avg_in(ds_system *s, const void *src, double *dst, size_t n, Buf &stage) {
     const size_t nb = n * elem_size(s);
@@ -681,7 +733,7 @@ int ds_destroy(ds_system *s) {
     cudaSetDevice(s->P.device);
     cudaStreamSynchronize(s->stream);
     void *ptrs[] = {s->X, s->xu, s->Rref, s->msd_part, s->msd_out, s->phase, s->units[0], s->units[1], s->ll[0], s->ll[1], s->bar, s->pcnt, s->half_off, s->Xcg, s->V1g, s->Fg, s->Lg,
-                    s->ap_units.p, s->st_a.p, s->st_b.p, s->st_c.p, s->avg.p, s->avg_sc.p};
+                    s->ap_units.p, s->st_a.p, s->st_b.p, s->st_c.p, s->avg.p, s->avg_sc.p, s->avg_xch.p};
     for (void *q : ptrs) if (q) cudaFree(q);
     (void)cudaGetLastError();
     delete s;
@@ -915,12 +967,17 @@ int ds_avg_step(ds_system *s, void *R, void *Nv, const void *phase, int32_t S, d
     DS_TRY(avg_sincos(s, phd, S));
     DS_TRY(avg_in(s, R, Rd, M, s->st_a));
     DS_TRY(avg_in(s, Nv, Nd, M, s->st_b));
-    // Heun: two launches per step, the update of a block of dumbbells done by the CTA that completes
-    // its right-hand sides (averaged.cuh)
-    ds::AvgUpdate P1{ds::AVG_PRED, dt, Rd, Nd, dR1, dN1, Rp, Np}, P2{ds::AVG_CORR, dt, Rd, Nd, dR1, dN1, Rd, Nd};
-    for (int64_t n = 0; n < n_steps; ++n) {
-        DS_TRY(launch_avg_rhs<double>(s, Rd, Nd, S, (double *)nullptr, (double *)nullptr, P1));
-        DS_TRY(launch_avg_rhs<double>(s, Rp, Np, S, (double *)nullptr, (double *)nullptr, P2));
+    // Heun.  Sizes of the paper (S up to a few thousand): one cooperative launch runs all steps on the device
+    // (avg_persist_kernel).  Larger S: two launches per step, the update of a block of dumbbells done by the CTA that
+    // completes its right-hand sides (avg_rhs_kernel).
+    bool persistent = false;
+    DS_TRY(avg_step_persistent(s, Rd, Nd, S, dt, n_steps, &persistent));
+    if (!persistent) {
+        ds::AvgUpdate P1{ds::AVG_PRED, dt, Rd, Nd, dR1, dN1, Rp, Np}, P2{ds::AVG_CORR, dt, Rd, Nd, dR1, dN1, Rd, Nd};
+        for (int64_t n = 0; n < n_steps; ++n) {
+            DS_TRY(launch_avg_rhs<double>(s, Rd, Nd, S, (double *)nullptr, (double *)nullptr, P1));
+            DS_TRY(launch_avg_rhs<double>(s, Rp, Np, S, (double *)nullptr, (double *)nullptr, P2));
+        }
     }
     bool host = false;
     DS_TRY(avg_out(s, Rd, R, M, s->st_a, &host));

@@ -600,7 +600,7 @@ def test_avg_step_parity_lattice(precision, tol):
 def test_avg_step_parity_729(precision):
     """The paper's largest lattice, 9 x 9 x 9, sites displaced by up to 5 (no close pairs: Eq. (9) is a
     far-field model), random directions and phases: 6 Heun steps from the state as rounded to the working precision;
-    every s block is a cluster of 8 CTAs and the CTA that adds their sums also applies the predictor / corrector."""
+    the device-resident kernel: 5 dumbbells per CTA, all steps in one launch."""
     S = 729
     g = np.arange(9) * 30.0
     jit, N, phi = _avg_case(S, 31, 10.0)
@@ -618,6 +618,43 @@ def test_avg_step_parity_729(precision):
         assert np.abs(Rg - Ro).max() <= 1e-12 * 250 and np.abs(Ng - No).max() <= 1e-12
     else:   # float32 output buffers: half an ulp of 250 is 1.5e-5
         assert np.abs(Rg - Ro).max() <= 2e-5 and np.abs(Ng - No).max() <= 1e-5
+
+
+@pytest.mark.parametrize("precision", [ds.F64, ds.F32])
+@pytest.mark.parametrize("S", [1, 2, 7, 147, 149, 301, 2500, 4097])
+def test_avg_step_device_resident_and_two_launch_paths(S, precision):
+    """ds_avg_step over its launch shapes: one dumbbell (no pair at all), fewer dumbbells than SMs (one per CTA), one more
+    than the SM count (two per CTA, a last CTA with one), odd S (an odd lane in the last FP32 pack), many dumbbells per CTA
+    (S = 2500: 17), and S = 4097, above the limit of the device-resident kernel (two launches per step through
+    avg_rhs_kernel).  5 Heun steps; a second call continues from the first (tags of the exchange buffers advance)."""
+    m = int(np.ceil(S ** (1 / 3)))
+    g_ = np.arange(m) * 30.0                      # jittered lattice as in Fig. 3 / 4: no close pairs (Eq. (9) is a far-field model)
+    jit, N, phi = _avg_case(S, 700 + S, 10.0)
+    R = np.stack(np.meshgrid(g_, g_, g_, indexing="ij"), -1).reshape(-1, 3)[:S] + jit
+    R = R.astype(NPDT[precision]).astype(np.float64); N = N.astype(NPDT[precision]).astype(np.float64)
+    p = oracle.Params(a=0.8, ell=9.0, lam=1.7, omega=5.5)
+    Ro, No = oracle.avg_step(R, N, phi, 40.0, 5, p)
+    with ds.System(1, precision=precision, a=p.a, ell=p.ell, lam=p.lam, omega=p.omega) as s:
+        Rd = torch.as_tensor(R, device="cuda").to(TDT[precision]); Nd = torch.as_tensor(N, device="cuda").to(TDT[precision])
+        l0 = s.launch_count()
+        s.avg_step(Rd, Nd, torch.as_tensor(phi, device="cuda"), S, 40.0, 5)
+        n_launch = s.launch_count() - l0
+        torch.cuda.synchronize()
+        Rg, Ng = Rd.cpu().numpy().astype(np.float64), Nd.cpu().numpy().astype(np.float64)
+        if precision == ds.F64:
+            s.avg_step(Rd, Nd, torch.as_tensor(phi, device="cuda"), S, 40.0, 3)     # 5 + 3 steps = 8 steps
+            torch.cuda.synchronize()
+            R8, N8 = oracle.avg_step(R, N, phi, 40.0, 8, p)
+            assert np.abs(Rd.cpu().numpy() - R8).max() <= 1e-11 * np.abs(R).max() + 1e-13
+            assert np.abs(Nd.cpu().numpy() - N8).max() <= 1e-12
+    # launches: sin/cos table + 2 widen + (1 resident | 2 per step) + 2 narrow
+    assert n_launch == (6 if S <= 4096 else 5 + 2 * 5)
+    scale = np.abs(R).max() + 1.0
+    if precision == ds.F64:
+        assert np.abs(Rg - Ro).max() <= 1e-12 * scale and np.abs(Ng - No).max() <= 1e-12
+    else:   # FP32 pair arithmetic (2e-5 of the right-hand sides, DESIGN.md section 4) and float32 output buffers
+        assert np.abs(Rg - Ro).max() <= 1e-4 * np.abs(Ro - R).max() + 1.2e-7 * scale
+        assert np.abs(Ng - No).max() <= 1e-4 * np.abs(No - N).max() + 3e-7
 
 
 # --------------------------------------------------------------------------------- pipelined step kernel (pipeline.cuh)
