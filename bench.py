@@ -39,7 +39,7 @@ FLOP_PER_PAIR = {"oseen": 27, "rpy": 34}
 FLOP_PER_PAIR_KERNEL = {"oseen": 27, "rpy": 33}
 # DRAM bytes (read + write) of one whole ds_step launch of the headline workload, from the ncu --set full capture of
 # the same command (profiles/r2_pipe_kernel_ncu_full.md): the path is ALU-bound and L2-resident
-NCU_DRAM_BYTES_PER_LAUNCH = {"f32": 321280, "f64": None}
+NCU_DRAM_BYTES_PER_LAUNCH = {"f32": 301568, "f64": None}
 # ALU peaks derived in DESIGN.md "Roofline": SMs x lanes x 2 x f_SM(max).  FP32: 128 lanes/SM.  FP64: the
 # DFMA rate of B200 is what ds_peak_probe measures; the nominal figure used is 64 lanes/SM.
 N_SM, F32_LANES, F64_LANES = 148, 128, 64
