@@ -16,6 +16,7 @@
 #include "../../include/ds_dev.h"
 #include "mobility.cuh"
 #include "pipeline.cuh"
+#include "small.cuh"
 #include "peak.cuh"
 #include "averaged.cuh"
 #include "state.cuh"
@@ -395,6 +396,37 @@ int launch_pipe_run(ds_system *s, long long n_steps) {
 #undef DS_PIPE
     }
     s->pcnt_base += (unsigned long long)s->n_cta * (unsigned long long)n_stage;
+    s->x_valid = true; s->xu_valid = true;
+    return DS_OK;
+}
+
+
+// RUN_STEP for small systems (S <= 32): one warp per system (small.cuh), any number of systems per launch
+template <typename T, int TENSOR, bool HEUN> int launch_small_v(ds_system *s, const ds::SmallArgs &A) {
+    const unsigned grid = (unsigned)((s->B + ds::SMALL_WARPS - 1) / ds::SMALL_WARPS);
+    ds::small_kernel<T, TENSOR, HEUN><<<grid, 32 * ds::SMALL_WARPS, 0, s->stream>>>(A);
+    CU_TRY(cudaGetLastError());
+    s->launches += 1;
+    return DS_OK;
+}
+
+int launch_small_run(ds_system *s, long long n_steps) {
+    ds::SmallArgs A;
+    memset(&A, 0, sizeof A);
+    A.S = s->S; A.B = s->B;
+    ds::RunArgs R;
+    memset(&R, 0, sizeof R);
+    fill_constants(s, R);
+    A.self_mob = R.self_mob; A.pre = R.pre; A.c1 = R.c1; A.c2 = R.c2; A.c1f = R.c1f; A.c2f = R.c2f;
+    A.t0 = R.t0; A.dt = R.dt; A.ell = R.ell; A.lambda = R.lambda; A.omega = R.omega; A.k0 = R.k0;
+    A.noise_amp = R.noise_amp; A.seed = R.seed;
+    A.n0 = s->n_host; A.n_steps = n_steps;
+    A.X = s->X; A.xu = s->xu; A.from_user = s->x_valid ? 0 : 1; A.phase = s->phase;
+    const bool heun = s->P.integrator == DS_HEUN, f64 = s->P.precision == DS_F64, rpy = s->P.tensor == DS_RPY;
+#define DS_SMALL(TT, TEN) (heun ? launch_small_v<TT, TEN, true>(s, A) : launch_small_v<TT, TEN, false>(s, A))
+    if (f64) DS_TRY(rpy ? DS_SMALL(double, ds::TENSOR_RPY) : DS_SMALL(double, ds::TENSOR_OSEEN));
+    else DS_TRY(rpy ? DS_SMALL(float, ds::TENSOR_RPY) : DS_SMALL(float, ds::TENSOR_OSEEN));
+#undef DS_SMALL
     s->x_valid = true; s->xu_valid = true;
     return DS_OK;
 }
@@ -1064,7 +1096,9 @@ int ds_batch_step(ds_system *s, int64_t n_steps) {
     int64_t left = n_steps;
     while (left > 0) {   // one launch runs up to MAX_STEPS_PER_LAUNCH steps entirely on the device
         const long long k = left < MAX_STEPS_PER_LAUNCH ? left : MAX_STEPS_PER_LAUNCH;
-        DS_TRY(s->use_pipe ? launch_pipe_run(s, k) : launch_state_run(s, ds::RUN_STEP, k, nullptr));
+        // small systems: a warp per system; a forced tiling (ds_set_tuning) keeps them on run_kernel (tests)
+        if (s->S <= ds::SMALL_MAX_S && s->tune_cta == 0) DS_TRY(launch_small_run(s, k));
+        else DS_TRY(s->use_pipe ? launch_pipe_run(s, k) : launch_state_run(s, ds::RUN_STEP, k, nullptr));
         s->n_host += k; left -= k;
     }
     return DS_OK;

@@ -175,16 +175,16 @@ __device__ __forceinline__ void red_release_gpu(unsigned long long *p, unsigned 
 // (second line of (3b): 2a^2/(24 pi mu r^3) (delta - 3 rr/r^2) = (1/8 pi mu)(1/r^3)[(2a^2/3) delta - 2a^2 rr/r^2]).
 // The common factor 1/(8 pi mu) is applied once per alpha in the epilogue.
 // FMA-pipe instruction count per pack: 3 sub + 3 (r^2) + 3 (r.F) + 2 + 6 = 17 (Oseen), 21 (RPY).
-template <typename T, int TENSOR, bool GUARD>
-__device__ __forceinline__ void pair_unit(const V2<T> *__restrict__ p, const typename Pack<T>::V (&xi)[QI][3],
-                                          typename Pack<T>::V (&acc)[QI][3], typename Pack<T>::V c1,
+template <typename T, int TENSOR, bool GUARD, int NA = QI>
+__device__ __forceinline__ void pair_unit(const V2<T> *__restrict__ p, const typename Pack<T>::V (&xi)[NA][3],
+                                          typename Pack<T>::V (&acc)[NA][3], typename Pack<T>::V c1,
                                           typename Pack<T>::V negc2) {
     typedef Pack<T> P;
     typedef typename P::V V;
     const V2<T> q0 = p[0], q1 = p[1], q2 = p[2];
     const V xj = q0.a, yj = q0.b, zj = q1.a, fx = q1.b, fy = q2.a, fz = q2.b;
 #pragma unroll
-    for (int k = 0; k < QI; ++k) {
+    for (int k = 0; k < NA; ++k) {
         const V dx = P::sub(xi[k][0], xj), dy = P::sub(xi[k][1], yj), dz = P::sub(xi[k][2], zj);
         const V r2 = P::fma(dz, dz, P::fma(dy, dy, P::mul(dx, dx)));
         const V ri = P::template rsq<GUARD>(r2);

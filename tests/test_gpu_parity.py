@@ -812,3 +812,34 @@ def test_step_state_in_global_memory_odd_S_batch():
     for b in range(w.B):
         Xo = oracle.step(X0[b], w.phase[b], 0.0, 0, 6, p)
         assert np.abs(out.cpu().numpy()[b] - Xo).max() <= 1e-10 * ELL
+
+
+# --------------------------------------------------------------------------------- small systems: one warp per system (small.cuh)
+@pytest.mark.parametrize("precision,tol", [(ds.F32, 1e-4), (ds.F64, 1e-10)])
+@pytest.mark.parametrize("S,B", [(1, 1), (2, 3), (3, 1), (5, 7), (8, 1), (17, 5), (32, 9)])
+def test_small_system_kernel_shapes(S, B, precision, tol):
+    """S <= 32 dumbbells run one warp per system: 32, 16, 8, 4, 2, 1 lanes per dumbbell (S = 1 ... 32, powers of two and
+    not), several systems per CTA and a ragged last CTA.  60 Heun steps over three calls, t0 != 0, against the oracle;
+    the same steps through run_kernel's one-CTA mode (forced tiling) agree to rounding."""
+    w = inputs.config5(B=B, S=S)
+    Xg, X0, p = gpu_steps(w, precision, 60, t0=0.1, chunks=[7, 1, 52])
+    for b in range(B):
+        Xo = oracle.step(X0[b], w.phase[b], 0.1, 0, 60, p)
+        assert np.abs(Xg[b] - Xo).max() <= tol * ELL
+    Xr, _, _ = pipe_steps(w, precision, [60], n_tiles=1, t0=0.1, pipeline=0)       # run_kernel, one CTA per system
+    assert np.abs(Xg - Xr).max() <= (1e-5 if precision == ds.F32 else 1e-11) * ELL
+
+
+@pytest.mark.parametrize("integrator", [ds.EULER, ds.HEUN])
+@pytest.mark.parametrize("tensor", [ds.OSEEN, ds.RPY])
+def test_small_system_kernel_integrators_tensors_noise(integrator, tensor):
+    """Euler / Heun, Oseen / RPY, k_B T > 0 (Philox increments drawn per lane), chunking invariance bit for bit, host-buffer
+    start."""
+    import dataclasses
+    w = inputs.config5(B=3, S=12)
+    Xa, X0, p = gpu_steps(w, ds.F64, 101, tensor, integrator, t0=0.25, kT=0.02, seed=0xABCDEF12345)
+    Xb, _, _ = gpu_steps(w, ds.F64, 101, tensor, integrator, t0=0.25, chunks=[1, 33, 3, 64], kT=0.02, seed=0xABCDEF12345)
+    assert np.array_equal(Xa, Xb)
+    for b in range(w.B):
+        Xo = oracle.step(X0[b], w.phase[b], 0.25, 0, 101, dataclasses.replace(p, system=b))
+        assert np.abs(Xa[b] - Xo).max() <= 1e-9 * ELL
