@@ -333,10 +333,12 @@ int setup_pipe(ds_system *s) {
                        (size_t)rows_max * ds::STATE_BYTES_PER_ROW;
     if (smem > (size_t)ds::SMEM_MAX) return DS_OK;
     if (s->pipe_mode < 0) {
-        // heuristic: the pipeline hides a stage's fixed cost (about 5.5 k cycles) behind the pair loop of the other half;
-        // it pays once a quarter of a stage's pair work is longer than that: iterations of the unsplit shape >= 16
+        // heuristic: the pipeline hides a stage's fixed cost behind the pair loop of the other half, but its own hand-over chain
+        // (tail -> release -> every CTA arrived -> bulk copy, about 7 k cycles, twice per stage through one service warp) bounds a
+        // stage from below at about 6.8 us.  Measured per stage, pipelined / one-pass: N = 1024: 6.9 / 4.9 us, 2048: 7.6 / 7.8,
+        // 3072: 10.5 / 11.8, 4096: 13.5 / 15.6.  Switch at 8 pair-loop iterations of the one-pass shape (N = 2048 on 128 CTAs).
         const int nq = (s->NQ + n - 1) / n, n_jg = ds::NT / nq;
-        if ((s->U + n_jg - 1) / n_jg < 16) return DS_OK;
+        if ((s->U + n_jg - 1) / n_jg < 8) return DS_OK;
     }
     if (s->half_off_cap < 2 * (n + 1)) {
         if (s->half_off) CU_TRY(cudaFree(s->half_off));
