@@ -403,6 +403,53 @@ int launch_pipe_run(ds_system *s, long long n_steps) {
 }
 
 
+// ds_mobility_apply through apply_kernel (pipeline.cuh) when every CTA owns at most 16 quads and the stream with its pad
+// units fits shared memory; *used says whether it ran.
+template <typename T, int TENSOR> int launch_apply_v(ds_system *s, const ds::ApplyArgs &A, size_t smem) {
+    auto kern = ds::apply_kernel<T, TENSOR>;
+    static SmemOptIn opt_in;
+    DS_TRY(opt_in.ensure((const void *)kern, s->P.device));
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof cfg);
+    cfg.gridDim = dim3((unsigned)A.n_cta); cfg.blockDim = dim3(32 * ds::PIPE_CW); cfg.dynamicSmemBytes = smem; cfg.stream = s->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    CU_TRY(cudaLaunchKernelEx(&cfg, kern, A));
+    s->launches += 1;
+    return DS_OK;
+}
+
+int apply_warp_shape(ds_system *s, const ds::RunArgs &R, const void *dpos, const void *dF, void *du, bool *used) {
+    *used = false;
+    if (s->pipe_mode == 0) return DS_OK;
+    const int nq_hi = (R.NQ + R.n_cta - 1) / R.n_cta, nq_lo = R.NQ / R.n_cta;
+    if (nq_hi > ds::PIPE_CW || nq_lo < 1) return DS_OK;
+    int cap = R.U;
+    for (int nq = nq_lo; nq <= nq_hi; ++nq)
+        for (int extra = 0; extra < 2; ++extra) {
+            if (extra && ds::PIPE_CW % nq == 0) continue;
+            const int n_jg = 32 * (ds::PIPE_CW / nq + extra), need = (R.U + n_jg - 1) / n_jg * n_jg;
+            cap = need > cap ? need : cap;
+        }
+    cap = (cap + 7) / 8 * 8;
+    const size_t smem = (size_t)cap * ds::UNIT_BYTES + (size_t)ds::PIPE_CW * 12 * sizeof(double);
+    if (smem > (size_t)ds::SMEM_MAX) return DS_OK;
+    ds::ApplyArgs A;
+    memset(&A, 0, sizeof A);
+    A.N = R.N; A.NQ = R.NQ; A.U = R.U; A.n_cta = R.n_cta; A.buf_units = cap;
+    A.self_mob = R.self_mob; A.pre = R.pre; A.c1 = R.c1; A.c2 = R.c2; A.c1f = R.c1f; A.c2f = R.c2f;
+    A.raw_pos = dpos; A.raw_F = dF; A.out_u = du;
+    const bool f64 = s->P.precision == DS_F64, rpy = s->P.tensor == DS_RPY;
+    int rc;
+    if (f64) rc = rpy ? launch_apply_v<double, ds::TENSOR_RPY>(s, A, smem) : launch_apply_v<double, ds::TENSOR_OSEEN>(s, A, smem);
+    else rc = rpy ? launch_apply_v<float, ds::TENSOR_RPY>(s, A, smem) : launch_apply_v<float, ds::TENSOR_OSEEN>(s, A, smem);
+    DS_TRY(rc);
+    *used = true;
+    return DS_OK;
+}
+
 // RUN_STEP for small systems (S <= 32): one warp per system (small.cuh), any number of systems per launch
 template <typename T, int TENSOR, bool HEUN> int launch_small_v(ds_system *s, const ds::SmallArgs &A) {
     const unsigned grid = (unsigned)((s->B + ds::SMALL_WARPS - 1) / ds::SMALL_WARPS);
@@ -1066,7 +1113,11 @@ int ds_mobility_apply(ds_system *s, const void *pos, const void *F, void *u, int
     A.out_u = du;
     A.probe = s->probe;
     const bool aligned = (((uintptr_t)dpos | (uintptr_t)dF) & 7u) == 0;   // the in-kernel pack reads 8-byte pairs
-    if (aligned && stream_resident(A.NQ, A.U, A.n_cta, A.buf_bytes)) {
+    bool warp_shape = false;
+    if (aligned && (s->tune_cta == 0 || s->pipe_mode == 1)) DS_TRY(apply_warp_shape(s, A, dpos, dF, du, &warp_shape));
+    if (warp_shape) {
+        // done: apply_kernel packed the user's arrays itself
+    } else if (aligned && stream_resident(A.NQ, A.U, A.n_cta, A.buf_bytes)) {
         A.raw_pos = dpos; A.raw_F = dF;
         A.unit_stride = (long long)U + ds::PAD_UNITS;
     } else {
@@ -1082,7 +1133,7 @@ int ds_mobility_apply(ds_system *s, const void *pos, const void *F, void *u, int
         A.unit_stride = n_units;
         A.units[0] = s->ap_units.p; A.units[1] = s->ap_units.p;
     }
-    DS_TRY(launch_run(s, A, dim3((unsigned)A.n_cta, 1), (size_t)A.buf_bytes + ds::BAR_BYTES, false, s->stream));
+    if (!warp_shape) DS_TRY(launch_run(s, A, dim3((unsigned)A.n_cta, 1), (size_t)A.buf_bytes + ds::BAR_BYTES, false, s->stream));
     if (!du_dev) {
         CU_TRY(cudaMemcpyAsync(u, du, nb, cudaMemcpyDeviceToHost, s->stream));
         CU_TRY(cudaStreamSynchronize(s->stream));

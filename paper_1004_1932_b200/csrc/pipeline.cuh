@@ -421,4 +421,115 @@ __global__ void __launch_bounds__(PIPE_NT, 1) pipe_kernel(const PipeArgs A) {
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------------
+// The stateless mobility apply (ds_mobility_apply: Eq. (1a) deterministic part with Eq. (3a,3b)) in the
+// thread shape of the pipelined kernel, one pass: the 16 warps of a CTA are dealt to its nq <= 16 quads (16 / nq or one more
+// each), all lanes of a warp hold the same 4 alpha-spheres and walk 32 consecutive units of the stream per iteration; the
+// split-beta sums meet in the fixed shuffle tree of warp_sum12 and in 12 numbers per warp of shared memory (run_kernel's
+// apply mode needs a 24 KB block-wide reduction instead).  Every CTA packs the user's [n][3] arrays into its own stream;
+// no inter-CTA dependency: a plain launch with programmatic dependent launch, any number of waves.
+struct ApplyArgs {
+    int N, NQ, U, n_cta;
+    int buf_units;                 // capacity of the stream buffer in units (pads included, multiple of 8)
+    double self_mob, pre, c1, c2;
+    float c1f, c2f;
+    const void *raw_pos, *raw_F;   // user arrays [N][3]
+    void *out_u;                   // [N][3]
+};
+
+template <typename T, int TENSOR>
+__global__ void __launch_bounds__(32 * PIPE_CW, 1) apply_kernel(const ApplyArgs A) {
+    typedef Pack<T> P;
+    typedef typename P::V V;
+    constexpr int W = P::W, NTH = 32 * PIPE_CW;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int c = blockIdx.x;
+    T *const scr = reinterpret_cast<T *>(smem_raw + (size_t)A.buf_units * UNIT_BYTES);   // [16][12]
+
+    const int q0 = (int)((long long)c * A.NQ / A.n_cta), q1 = (int)((long long)(c + 1) * A.NQ / A.n_cta);
+    const int nq = q1 - q0;                                            // 1 .. 16 (host)
+    const long long r0 = 4LL * q0;
+    const int nrows = (int)((A.N - r0) < 4 * nq ? (A.N - r0) : 4 * nq);
+    // this warp's place: quad q gets mb + (q < mr) warps
+    const int mb = PIPE_CW / nq, mr = PIPE_CW % nq;
+    const int wq = warp < mr * (mb + 1) ? warp / (mb + 1) : mr + (warp - mr * (mb + 1)) / mb;
+    const int quad = wq, m = mb + (quad < mr ? 1 : 0);
+    const int sub = warp - (quad * mb + (quad < mr ? quad : mr));
+    const int n_jg = 32 * m;
+
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    // the warp's alpha rows, straight from the user's array (in flight while the stream is packed)
+    T xq[12];
+#pragma unroll
+    for (int k = 0; k < QI; ++k) {
+        const long long i = r0 + 4 * quad + k;
+#pragma unroll
+        for (int cc = 0; cc < 3; ++cc) xq[3 * k + cc] = i < A.N ? __ldg(reinterpret_cast<const T *>(A.raw_pos) + 3 * i + cc) : P::dummy();
+    }
+    {   // every CTA packs the whole stream for itself (units behind the last sphere are far-away zero-force dummies);
+        // CTAs start at different units so that they do not read L2 in a convoy
+        typedef typename std::conditional<sizeof(T) == 4, float4, double2>::type Q;
+        const int up = A.buf_units;
+        int u = tid + (int)(((long long)c * up) / A.n_cta);
+        for (int k = tid; k < up; k += NTH, u += NTH) {
+            u = u >= up ? u - up : u;
+            pack_unit(reinterpret_cast<Q *>(smem_raw) + 3 * u, reinterpret_cast<const T *>(A.raw_pos), reinterpret_cast<const T *>(A.raw_F), u, A.N);
+        }
+    }
+    __syncthreads();
+    const V c1 = P::bc(sizeof(T) == 4 ? (T)A.c1f : (T)A.c1), negc2 = P::bc(sizeof(T) == 4 ? (T)(-A.c2f) : (T)(-A.c2));
+    V xi[QI][3], acc[QI][3];
+#pragma unroll
+    for (int k = 0; k < QI; ++k) {
+        xi[k][0] = P::bc(xq[3 * k]); xi[k][1] = P::bc(xq[3 * k + 1]); xi[k][2] = P::bc(xq[3 * k + 2]);
+        acc[k][0] = acc[k][1] = acc[k][2] = P::bc(T(0));
+    }
+    {
+        const int its = (A.U + n_jg - 1) / n_jg;
+        const int its_w = its - ((its > 0 && (its - 1) * n_jg + 32 * sub >= A.U) ? 1 : 0);   // all 32 units behind the stream
+        const int own0 = (int)(r0 / W), own1 = own0 + (nrows + W - 1) / W;                   // units that hold own rows
+        int g_lo = own0 / n_jg, g_hi = (own1 - 1) / n_jg + 1;
+        g_lo = g_lo < its_w ? g_lo : its_w; g_hi = g_hi < its_w ? g_hi : its_w;
+        const V2<T> *p = reinterpret_cast<const V2<T> *>(smem_raw) + 3 * (32 * sub + lane);
+        const int stride = 3 * n_jg;
+        int it = 0;
+#pragma unroll 1
+        for (; it < g_lo; ++it, p += stride) pair_unit<T, TENSOR, false>(p, xi, acc, c1, negc2);
+#pragma unroll 1
+        for (; it < g_hi; ++it, p += stride) {
+            const int u0 = it * n_jg + 32 * sub;
+            if (u0 < own1 && u0 + 32 > own0) pair_unit<T, TENSOR, true>(p, xi, acc, c1, negc2);
+            else pair_unit<T, TENSOR, false>(p, xi, acc, c1, negc2);
+        }
+#pragma unroll 1
+        for (; it < its_w; ++it, p += stride) pair_unit<T, TENSOR, false>(p, xi, acc, c1, negc2);
+    }
+    {
+        T v[12], sm3[3];
+#pragma unroll
+        for (int k = 0; k < QI; ++k)
+#pragma unroll
+            for (int cc = 0; cc < 3; ++cc) v[3 * k + cc] = P::hsum(acc[k][cc]);
+        warp_sum12<T>(v, lane, sm3);
+        if ((lane & 7) == 0) {
+            T *dst = scr + warp * 12 + 3 * (lane >> 3);
+            dst[0] = sm3[0]; dst[1] = sm3[1]; dst[2] = sm3[2];
+        }
+    }
+    __syncthreads();
+    // a2 + a3: the warps of a quad in order, self term Eq. (3a), 1/(8 pi mu); one output element per thread
+    for (int e = tid; e < 3 * nrows; e += NTH) {
+        const int rl = e / 3, cc = e - 3 * rl, qd = rl >> 2, k = rl & 3;
+        const int mq = mb + (qd < mr ? 1 : 0);
+        const T *sp = scr + (qd * mb + (qd < mr ? qd : mr)) * 12 + 3 * k + cc;
+        T sacc = T(0);
+        for (int j = 0; j < mq; ++j) sacc += sp[12 * j];
+        const size_t gi = (size_t)3 * r0 + e;
+        const double Fi = (double)reinterpret_cast<const T *>(A.raw_F)[gi];
+        reinterpret_cast<T *>(A.out_u)[gi] = (T)(A.self_mob * Fi + A.pre * (double)sacc);
+    }
+}
+
 }  // namespace ds

@@ -38,11 +38,13 @@ def dev(x, precision):
     return torch.as_tensor(np.ascontiguousarray(x, dtype=NPDT[precision]), device="cuda")
 
 
-def gpu_apply(X, F, precision, tensor, a=1.0, eta=1.0, n_tiles=0, host=False):
+def gpu_apply(X, F, precision, tensor, a=1.0, eta=1.0, n_tiles=0, host=False, pipeline=None):
     n = X.shape[0]
     with ds.System(1, precision=precision, tensor=tensor, a=a, eta=eta) as s:
         if n_tiles:
             s.set_tuning(n_tiles)
+        if pipeline is not None:
+            s.set_pipeline(pipeline)
         if host:
             Xh = np.ascontiguousarray(X, dtype=NPDT[precision])
             Fh = np.ascontiguousarray(F, dtype=NPDT[precision])
@@ -99,6 +101,25 @@ def test_apply_parity_forced_tiles(n_tiles, precision):
     X, F = inputs.apply_case(1536, 21, 22)
     u = gpu_apply(X, F, precision, ds.RPY, n_tiles=n_tiles)
     assert rel_l2(u, oracle_apply(X, F, precision, ds.RPY)) <= TOL[precision]
+
+
+@pytest.mark.parametrize("precision", [ds.F32, ds.F64])
+@pytest.mark.parametrize("tensor", [ds.OSEEN, ds.RPY])
+@pytest.mark.parametrize("N,n_tiles", [(1536, 24), (1536, 35), (1536, 100), (1536, 384), (1537, 97), (130, 33), (6, 1), (1, 1), (4096, 0), (8192, 0)])
+def test_apply_warp_shaped_kernel(N, n_tiles, tensor, precision):
+    """apply_kernel (the stateless apply in the thread shape of the pipelined kernel) under forced tilings: 16 ... 1 quads per
+    CTA (1 ... 16 warps per quad, uneven deals like 11 quads on 16 warps), odd N (a half-filled last unit that holds an own
+    sphere), tiny N, and the library's own shapes at N = 4096 and 8192; per row against the oracle; the one-pass run_kernel on
+    the same tiling agrees within the tolerance; bitwise reproducible."""
+    X, F = inputs.ragged_case(N, 900 + N)
+    ref = oracle_apply(X, F, precision, tensor)
+    u = gpu_apply(X, F, precision, tensor, n_tiles=n_tiles, pipeline=1)
+    assert np.isfinite(u).all()
+    assert rel_l2(u, ref) <= TOL[precision]
+    assert np.abs(u - ref).max() <= 20 * TOL[precision] * np.sqrt(np.mean(ref ** 2))
+    u1 = gpu_apply(X, F, precision, tensor, n_tiles=n_tiles, pipeline=0)
+    assert rel_l2(u1, ref) <= TOL[precision]
+    assert np.array_equal(u, gpu_apply(X, F, precision, tensor, n_tiles=n_tiles, pipeline=1))
 
 
 @pytest.mark.parametrize("precision", [ds.F32, ds.F64])
