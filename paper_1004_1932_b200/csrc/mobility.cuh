@@ -670,12 +670,15 @@ __global__ void __launch_bounds__(NT, 1) run_kernel(const RunArgs A) {
                 const int its = sg.y & 0xffffff;
                 const int its_mine = its - ((sg.y >> 30) && skip_tail ? 1 : 0);
                 if (sg.w != 0) {
-                    // iterations that hold the CTA's own rows: a warp takes the guarded variant (r = 0 excluded)
-                    // only if one of its lanes reads an own unit in that iteration
+                    // iterations that hold the CTA's own rows: a warp takes the guarded variant (r = 0 excluded) only if
+                    // one of its lanes reads a unit of ITS OWN quad in that iteration (alpha == beta is possible nowhere
+                    // else; with many rows per CTA, e.g. 256 at B = 64 x N = 512, half the stream is "own" units)
                     int u = (sg.w - 1) * n_jg + jgr;
+                    constexpr unsigned UPQ = QI / W;                       // units of a quad
+                    const int uq0 = d0 + ith * (int)UPQ;                   // first unit of this thread's quad
 #pragma unroll 1
                     for (int r = 0; r < its; ++r, p += stride, u += n_jg) {
-                        const bool own = __any_sync(0xffffffffu, active && u >= d0 && u < d1);
+                        const bool own = __any_sync(0xffffffffu, active && (unsigned)(u - uq0) < UPQ);
                         if (active && r < its_mine) {
                             if (own) pair_unit<T, TENSOR, true>(p, xi, acc, c1, negc2);
                             else pair_unit<T, TENSOR, false>(p, xi, acc, c1, negc2);
