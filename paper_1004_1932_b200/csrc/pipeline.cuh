@@ -10,18 +10,18 @@
 // How.  The rows of a CTA are cut into two halves A and B (whole quads), and a stage into two passes:
 //     pass A: alpha in half A  x  all beta        pass B: alpha in half B  x  all beta
 // The beta-stream of a stage is laid out as two regions, region h = the half-h rows of every CTA (a fixed order, so
-// sums stay deterministic).  When pass A ends, the sums of the half-A rows are complete: a 17th "service" warp finishes
-// them (self term, integrator, Eq. (4), publish into region A of the NEXT stage's stream) while the 16 compute warps are
-// already in pass B.  Likewise the half-B rows are finished during pass A of the next stage, which starts on region A
+// sums stay deterministic).  When pass A ends, the sums of the half-A rows are complete: a "service" warpgroup (warps
+// 16-19) finishes them (self term, integrator, Eq. (4), publish into region A of the NEXT stage's stream) while the 16
+// compute warps are already in pass B.  Likewise the half-B rows are finished during pass A of the next stage, which starts on region A
 // of the new stream (published by every CTA half a stage ago) and reaches region B long after it has landed.  The
-// service warp also prefetches each region into shared memory with one TMA bulk copy as soon as (a) every CTA has
+// lead service warp also prefetches each region into shared memory with one TMA bulk copy as soon as (a) every CTA has
 // published it (one arrival counter per region and system, release/acquire at gpu scope) and (b) every compute warp of
 // this CTA has finished with the region's previous content (mbarrier).  No block-wide barrier inside the step loop.
 //
 // Thread shape of a pass over nq quads: m = 16 / nq warps per quad, lanes = 32 m beta-groups; all lanes of a warp hold
 // the same 4 alpha-spheres (loads of the alpha rows are broadcasts) and read 32 consecutive units of the stream
 // (48-byte stride: conflict-free LDS.128).  At the end of a pass a warp adds its 32 lanes' partial sums with a fixed
-// shuffle tree (12 values: 18 SHFL) and leaves 12 numbers in shared memory; the service warp adds the m warps of a
+// shuffle tree (12 values: 18 SHFL) and leaves 12 numbers in shared memory; the service warpgroup adds the m warps of a
 // quad in a fixed order.  No atomics anywhere: results are bitwise reproducible and independent of how the steps are
 // split over launches.
 #pragma once
