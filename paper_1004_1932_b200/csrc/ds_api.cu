@@ -308,7 +308,7 @@ int setup_pipe(ds_system *s) {
         const int nq = (int)(q1 - q0);
         const long long left = (long long)s->N - 4 * q0;
         const int nrows = (int)(left < 4LL * nq ? left : 4LL * nq);
-        const int nqA = (nq + 1) / 2, nqB = nq - nqA;
+        const int nqA = ds::pipe_split(nq), nqB = nq - nqA;
         const int rowsA = 4 * nqA < nrows ? 4 * nqA : nrows, rowsB = nrows - rowsA;
         off[c + 1] = off[c] + rowsA / W;
         off[(n + 1) + c + 1] = off[(n + 1) + c] + rowsB / W;

@@ -39,6 +39,12 @@ constexpr int PIPE_BAR_BYTES = 128;              // 8 mbarriers
 constexpr int PIPE_SCR_BYTES = 2 * PIPE_CW * 12 * 8;   // warp sums of the two passes, [2][16][12] T
 constexpr int PIPE_TAB_BYTES = 2 * PIPE_CW * 3 * 16;   // per pass and warp: its place in the pass and its loop bounds (stage-invariant)
 
+// quads of a CTA that form half A (the rest is half B)
+#ifndef PIPE_SPLIT_EXPR
+#define PIPE_SPLIT_EXPR ((nq + 1) >> 1)
+#endif
+__host__ __device__ inline int pipe_split(int nq) { return PIPE_SPLIT_EXPR; }
+
 struct PipeArgs {
     int N, NQ, n_cta, b0;
     long long unit_stride;        // units per system in the streams
@@ -119,7 +125,7 @@ __global__ void __launch_bounds__(PIPE_NT, 1) pipe_kernel(const PipeArgs A) {
     const long long r0 = 4LL * q0;
     const int nrows = (int)((A.N - r0) < 4 * nq ? (A.N - r0) : 4 * nq);
     const int nd = nrows >> 1;
-    const int nqA = (nq + 1) >> 1;
+    const int nqA = pipe_split(nq);
     const int rowsA = 4 * nqA < nrows ? 4 * nqA : nrows, rowsB = nrows - rowsA;
     const int *const ho0 = A.half_off, *const ho1 = A.half_off + (A.n_cta + 1);
     const int ownA = ho0[c], ownB = ho1[c];                           // first own unit inside region 0 / 1
