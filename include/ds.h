@@ -63,7 +63,8 @@ typedef enum {
     DS_ERR_CUDA = -3,          /* a CUDA runtime call failed; ds_last_cuda_error() says which    */
     DS_ERR_STATE = -4,         /* call needs a state (ds_set_state) or a different n_batch       */
     DS_ERR_NO_DEVICE = -5,     /* no sm_100-class CUDA device                                    */
-    DS_ERR_ALLOC = -6          /* host or device allocation failed                               */
+    DS_ERR_ALLOC = -6,         /* host or device allocation failed                               */
+    DS_ERR_TOO_LARGE = -7      /* the problem exceeds a fixed capacity stated at the call (ds_msd_static) */
 } ds_status;
 
 typedef struct {
@@ -147,6 +148,26 @@ int ds_velocity(ds_system *s, void *V);
 int ds_dumbbell_coords(ds_system *s, void *R, void *Nv);
 int ds_msd_set_reference(ds_system *s);
 int ds_msd(ds_system *s, double *msd);
+
+/* Eq. (13) for callers that may not allocate: CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc.  The same two kernels as ds_msd (per-chunk partial sums, then one block adds them in a fixed order), but the
+ * partial sums live in a file-scope `static __device__` array of DS_MSD_STATIC_MAX_PARTIALS doubles (128 KB, held by every
+ * GPU that loads the library until the process exits) instead of a buffer ds_msd_set_reference allocates.  The call needs
+ * no ds_system and calls no cudaMalloc, cudaFree or allocating library routine (its one-time set-up per device is a
+ * cudaGetSymbolAddress).
+ *   X     device pointer, FP64 sphere positions [W][2 S][3] (spheres 2s, 2s + 1 = dumbbell s, as in ds_set_state)
+ *   Rref  device pointer, FP64 reference centres R^s(0; w) [W][S][3]
+ *   S, W  dumbbells per system (>= 1), systems (>= 1); W * ceil(S / 256) <= DS_MSD_STATIC_MAX_PARTIALS, else DS_ERR_TOO_LARGE
+ *   msd   device pointer to one double, written by the second kernel (read it after the stream has reached that point)
+ *   stream  a cudaStream_t of `device` (NULL = default stream); device = CUDA device ordinal, made current by the call
+ * Asynchronous.  Inputs are read, *msd is written, nothing else of the caller's is touched.  Every partial sum a call reads
+ * it has written itself (nothing has to start at zero, the array keeps the last call's contents otherwise).  ALL calls on a
+ * device share the one array: calls that overlap on the GPU (different streams, no ordering between them) race and give
+ * wrong sums; calls in one stream, or ordered by events, are safe.
+ * DS_ERR_NULL for a NULL X, Rref or msd; DS_ERR_INVALID_PARAM for S < 1, W < 1 or an unknown device; DS_ERR_TOO_LARGE beyond
+ * the limit (nothing is launched); DS_ERR_NO_DEVICE / DS_ERR_CUDA as elsewhere.                                         */
+#define DS_MSD_STATIC_MAX_PARTIALS 16384
+int ds_msd_static(const double *X, const double *Rref, int32_t S, int32_t W, double *msd, void *stream, int32_t device);
 
 /* Stroke-averaged far-field model, Eq. (9a)-(9d): the paper's comparison model, a second O(S^2) pair sum
  * over dumbbells (centres R, unit directions Nv, stroke phases).  Stateless: S is any dumbbell count >= 1; a, ell, lambda,

@@ -724,6 +724,32 @@ int materialize_x(ds_system *s) {
 }  // namespace
 
 // =================================================================================================
+// ---------------------------------------------------------------------------------------------------------------------
+// ds_msd_static: Eq. (13) with no allocation.  The partial sums of msd_partial_kernel live in this file-scope array (one
+// copy per GPU that loads the library, until exit).  In host code `msd_static_partials` is only a stand-in for the
+// symbol, NOT a device address: the kernels get the pointer cudaGetSymbolAddress returns, looked up once per device with
+// that device current.
+static __device__ __align__(256) double msd_static_partials[DS_MSD_STATIC_MAX_PARTIALS];
+
+namespace {
+constexpr int MSD_STATIC_MAX_DEVICES = 64;
+std::mutex msd_static_mu;
+double *msd_static_ptr[MSD_STATIC_MAX_DEVICES] = {nullptr};
+
+// device address of msd_static_partials on `device`, which must be current
+int msd_static_address(int device, double **out) {
+    std::lock_guard<std::mutex> lock(msd_static_mu);
+    if (msd_static_ptr[device] == nullptr) {
+        double *p = nullptr;
+        CU_TRY(cudaGetSymbolAddress((void **)&p, msd_static_partials));
+        if (p == nullptr) return DS_ERR_CUDA;
+        msd_static_ptr[device] = p;
+    }
+    *out = msd_static_ptr[device];
+    return DS_OK;
+}
+}  // namespace
+
 extern "C" {
 
 const char *ds_version(void) { return "paper_1004_1932_b200 0.1 (sm_100a)"; }
@@ -739,6 +765,7 @@ const char *ds_strerror(int code) {
         case DS_ERR_STATE: return "call not valid in the system's current state";
         case DS_ERR_NO_DEVICE: return "no sm_100-class CUDA device";
         case DS_ERR_ALLOC: return "allocation failed";
+        case DS_ERR_TOO_LARGE: return "problem exceeds the fixed capacity of this entry point";
         default: return "unknown error";
     }
 }
@@ -1175,6 +1202,26 @@ int ds_step(ds_system *s, int64_t n_steps) {
     if (!s) return DS_ERR_NULL;
     if (s->B != 1) return DS_ERR_STATE;
     return ds_batch_step(s, n_steps);
+}
+
+int ds_msd_static(const double *X, const double *Rref, int32_t S, int32_t W, double *msd, void *stream, int32_t device) {
+    if (!X || !Rref || !msd) return DS_ERR_NULL;
+    if (S < 1 || W < 1) return DS_ERR_INVALID_PARAM;
+    const long long n_chunk = ((long long)S + 255) / 256;
+    if ((long long)W * n_chunk > DS_MSD_STATIC_MAX_PARTIALS || W > 65535) return DS_ERR_TOO_LARGE;   // W is also a grid y extent
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { (void)cudaGetLastError(); return DS_ERR_NO_DEVICE; }
+    if (device < 0 || device >= ndev || device >= MSD_STATIC_MAX_DEVICES) return DS_ERR_INVALID_PARAM;
+    CU_TRY(cudaSetDevice(device));
+    double *partial = nullptr;
+    DS_TRY(msd_static_address(device, &partial));
+    cudaStream_t st = (cudaStream_t)stream;
+    // every partial the second kernel reads is written by the first: nothing in the shared array has to start at zero
+    ds::msd_partial_kernel<<<dim3((unsigned)n_chunk, (unsigned)W), 256, 0, st>>>(X, Rref, S, partial);
+    CU_TRY(cudaGetLastError());
+    ds::msd_final_kernel<<<1, 256, 0, st>>>(partial, W, S, (int)n_chunk, msd);
+    CU_TRY(cudaGetLastError());
+    return DS_OK;
 }
 
 }  // extern "C"

@@ -18,11 +18,12 @@ OSEEN, RPY = 0, 1
 EULER, HEUN = 0, 1
 
 OK = 0
-ERR_INVALID_PARAM, ERR_NULL, ERR_CUDA, ERR_STATE, ERR_NO_DEVICE, ERR_ALLOC = -1, -2, -3, -4, -5, -6
+ERR_INVALID_PARAM, ERR_NULL, ERR_CUDA, ERR_STATE, ERR_NO_DEVICE, ERR_ALLOC, ERR_TOO_LARGE = -1, -2, -3, -4, -5, -6, -7
+MSD_STATIC_MAX_PARTIALS = 16384
 
 # every symbol include/ds.h declares (tests check that the built library exports all of them)
 SYMBOLS = ["ds_create", "ds_destroy", "ds_set_stream", "ds_set_state", "ds_get_state", "ds_forces",
-           "ds_mobility_apply", "ds_step", "ds_batch_step", "ds_velocity", "ds_dumbbell_coords", "ds_msd_set_reference", "ds_msd", "ds_avg_rhs", "ds_avg_step", "ds_strerror", "ds_last_cuda_error", "ds_version"]
+           "ds_mobility_apply", "ds_step", "ds_batch_step", "ds_velocity", "ds_dumbbell_coords", "ds_msd_set_reference", "ds_msd", "ds_msd_static", "ds_avg_rhs", "ds_avg_step", "ds_strerror", "ds_last_cuda_error", "ds_version"]
 # development / measurement hooks (include/ds_dev.h)
 DEV_SYMBOLS = ["ds_set_tuning", "ds_set_probe", "ds_launch_count", "ds_peak_probe", "ds_set_pipeline", "ds_pipeline_active"]
 
@@ -70,6 +71,7 @@ def lib():
         L.ds_avg_step.argtypes = [vp, vp, vp, vp, i32, dbl, i64]
         L.ds_msd_set_reference.argtypes = [vp]
         L.ds_msd.argtypes = [vp, ctypes.POINTER(dbl)]
+        L.ds_msd_static.argtypes = [vp, vp, i32, i32, vp, vp, i32]
         L.ds_set_tuning.argtypes = [vp, i32]
         L.ds_set_probe.argtypes = [vp, vp]
         L.ds_set_pipeline.argtypes = [vp, i32]
@@ -115,6 +117,13 @@ def _ptr(x):
 def _check(code, where):
     if code != OK:
         raise DsError(code, where)
+
+
+def msd_static(X, Rref, S, W, out, stream=None, device=0):
+    """ds_msd_static: Eq. (13) from device arrays X [W][2S][3], Rref [W][S][3] (FP64) into the device double `out`;
+    allocates nothing (scratch = a static device array shared by all calls: do not overlap calls on the GPU)."""
+    _check(lib().ds_msd_static(_ptr(X), _ptr(Rref), int(S), int(W), _ptr(out), ctypes.c_void_p(stream or 0), int(device)),
+           "ds_msd_static")
 
 
 class System:
