@@ -172,7 +172,8 @@ def time_steps(torch, ds, w, precision, tensor, n_steps, warmup, ranks=None, sam
         t = np.array([a.elapsed_time(b) * 1e-3 for a, b in ev])
         info = {"repeats": reps, "warmup_launches": wl, "warmup_device_ms": warm * 1e3,
                 "ms_per_step_min": 1e3 * t.min() / n_steps, "ms_per_step_max": 1e3 * t.max() / n_steps,
-                "timed_region_ms": 1e3 * t.sum(), "pipelined_kernel": bool(s.pipeline_active())}
+                "timed_region_ms": 1e3 * t.sum(), "pipelined_kernel": s.pipeline_active() == 1,
+                "step_kernel": {0: "small" if w.S <= 32 else "one-pass", 1: "pipelined", 2: "cluster"}[s.pipeline_active()]}
         return float(np.median(t)), int(launches), info
 
 
@@ -438,7 +439,7 @@ def extras(torch, ds, inputs, w, args, precision, tensor):
         t, _, info = time_steps(torch, ds, wc, pr, ds.RPY, nst, 64)
         cfgs[name] = {"timesteps_per_s": nst / t, "pairs_per_s": nst * 2 * pairs_per_apply(wc.N, wc.B) / t,
                       "us_per_stage": 1e6 * t / (2 * nst), "steps_per_launch": nst, "repeats": info["repeats"],
-                      "pipelined_kernel": info["pipelined_kernel"]}
+                      "step_kernel": info["step_kernel"]}
     extra["configs_rpy_heun"] = cfgs
     extra["avg_model_eq9"] = avg_model_extra(torch, ds)
     extra["cold_l2"] = {"ms_per_step": 1e3 * time_steps_cold_l2(torch, ds, w, precision, tensor, 30),

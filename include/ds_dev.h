@@ -33,7 +33,10 @@ int ds_peak_probe(int32_t precision, int32_t device, double *flops_per_s);
  * (mobility.cuh), 1 = the pipelined two-pass kernel (pipeline.cuh) whenever the launch shape allows it (several CTAs per
  * system, each half of a CTA's rows at most 16 quads, streams resident in shared memory).  Both kernels advance the same
  * equations; they differ in the order of the split-beta sums, i.e. in the last bits.
- * ds_pipeline_active: 1 if the next ds_step would use the pipelined kernel.                                          */
+ * Ensembles (n_batch >= 2) whose systems can each take one thread-block cluster (cluster.cuh: all clusters resident at once
+ * and filling at least 3/4 of the SMs) use the cluster kernel unless mode is 0.
+ * ds_pipeline_active: the kernel the next ds_step / ds_batch_step would use: 0 = one-pass (or, for S <= 32, the
+ * warp-per-system kernel), 1 = pipelined two-pass, 2 = cluster kernel.                                                   */
 int ds_set_pipeline(ds_system *s, int32_t mode);
 int ds_pipeline_active(const ds_system *s);
 

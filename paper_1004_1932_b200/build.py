@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libds.so")
 SOURCES = ["ds_api.cu"]
-HEADERS = ["pack.cuh", "noise.cuh", "averaged.cuh", "mobility.cuh", "pipeline.cuh", "small.cuh", "state.cuh", "peak.cuh",
+HEADERS = ["pack.cuh", "noise.cuh", "averaged.cuh", "mobility.cuh", "pipeline.cuh", "small.cuh", "cluster.cuh", "state.cuh", "peak.cuh",
            os.path.join("..", "..", "include", "ds.h"), os.path.join("..", "..", "include", "ds_dev.h")]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "--shared", "-Xcompiler", "-fPIC"]

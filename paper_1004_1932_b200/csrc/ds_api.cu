@@ -17,6 +17,7 @@
 #include "mobility.cuh"
 #include "pipeline.cuh"
 #include "small.cuh"
+#include "cluster.cuh"
 #include "peak.cuh"
 #include "averaged.cuh"
 #include "state.cuh"
@@ -101,6 +102,10 @@ struct ds_system {
     // dominates a stage
     int pipe_mode = -1;                         // -1 = library heuristic, 0 = never, 1 = whenever the shape allows it
     bool use_pipe = false;
+    int cl_cs = 0;                              // > 0: cluster_kernel with this many CTAs per system (cluster.cuh)
+    int cl_buf_units[2] = {0, 0}, cl_rows_max = 0, cl_slots_max = 0;
+    int cl_half_off[2][ds::CL_MAX_CS + 1] = {};
+    size_t cl_smem = 0;
     int *half_off = nullptr;                    // device table [2][n_cta + 1]
     int half_off_cap = 0;
     int reg_units[2] = {0, 0}, pbuf_units[2] = {0, 0}, rows_max = 0;
@@ -447,6 +452,120 @@ int apply_warp_shape(ds_system *s, const ds::RunArgs &R, const void *dpos, const
     else rc = rpy ? launch_apply_v<float, ds::TENSOR_RPY>(s, A, smem) : launch_apply_v<float, ds::TENSOR_OSEEN>(s, A, smem);
     DS_TRY(rc);
     *used = true;
+    return DS_OK;
+}
+
+// the cluster kernel variant a system uses
+const void *cluster_kernel_of(const ds_system *s) {
+    const bool heun = s->P.integrator == DS_HEUN, f64 = s->P.precision == DS_F64, rpy = s->P.tensor == DS_RPY;
+#define DS_CLK(TT, TEN) (heun ? (const void *)ds::cluster_kernel<TT, TEN, true> : (const void *)ds::cluster_kernel<TT, TEN, false>)
+    if (f64) return rpy ? DS_CLK(double, ds::TENSOR_RPY) : DS_CLK(double, ds::TENSOR_OSEEN);
+    return rpy ? DS_CLK(float, ds::TENSOR_RPY) : DS_CLK(float, ds::TENSOR_OSEEN);
+#undef DS_CLK
+}
+
+// Shared-memory layout of the cluster kernel for cs CTAs per system; false if a half has too many quads or it does not fit.
+bool cluster_layout(ds_system *s, int cs) {
+    const int W = s->W;
+    int rows_max = 0, slots = 1, njg_max = 32;
+    s->cl_half_off[0][0] = s->cl_half_off[1][0] = 0;
+    for (int c = 0; c < cs; ++c) {
+        const long long q0 = (long long)c * s->NQ / cs, q1 = (long long)(c + 1) * s->NQ / cs;
+        const int nq = (int)(q1 - q0);
+        const long long left = (long long)s->N - 4 * q0;
+        const int nrows = (int)(left < 4LL * nq ? left : 4LL * nq);
+        const int nqA = ds::pipe_split(nq), nqB = nq - nqA;
+        const int rowsA = 4 * nqA < nrows ? 4 * nqA : nrows, rowsB = nrows - rowsA;
+        if (nqA > ds::CL_CW * ds::CL_MAX_QW) return false;
+        rows_max = rows_max > 4 * nq ? rows_max : 4 * nq;
+        for (int h = 0; h < 2; ++h) {
+            int QW, m;
+            ds::cluster_pass_shape(h == 0 ? nqA : nqB, QW, m);
+            const int sl = (h == 0 ? nqA : nqB) * m, njg = (32 / QW) * m;
+            slots = slots > sl ? slots : sl;
+            njg_max = njg_max > njg ? njg_max : njg;
+        }
+        s->cl_half_off[0][c + 1] = s->cl_half_off[0][c] + rowsA / W;
+        s->cl_half_off[1][c + 1] = s->cl_half_off[1][c] + rowsB / W;
+    }
+    size_t smem = ds::CL_BAR_BYTES + ds::CL_TAB_BYTES + (size_t)2 * slots * 12 * 8 + (size_t)rows_max * ds::STATE_BYTES_PER_ROW;
+    for (int h = 0; h < 2; ++h) {
+        s->cl_buf_units[h] = (s->cl_half_off[h][cs] + njg_max + 7) / 8 * 8;
+        smem += 2 * (size_t)s->cl_buf_units[h] * ds::UNIT_BYTES;
+    }
+    if (smem > (size_t)ds::SMEM_MAX) return false;
+    s->cl_rows_max = rows_max; s->cl_slots_max = slots; s->cl_smem = smem;
+    return true;
+}
+
+// Cluster step kernel (cluster.cuh) for ensembles: one thread-block cluster of cs CTAs per system, cs the largest of 8, 4, 2
+// for which all B clusters are resident at once (cudaOccupancyMaxActiveClusters: a cluster lives inside one GPC, so this is
+// fewer than SMs / cs).  Taken when those clusters fill at least 3/4 of the SMs (B = 64: cs = 2, 128 of 148), a CTA owns at
+// least a quad per warp, every half of a CTA has at most 16 * 8 quads, and two copies of the stream plus the state fit
+// shared memory.
+int setup_cluster(ds_system *s) {
+    s->cl_cs = 0;
+    if (s->pipe_mode == 0 || s->tune_cta != 0 || s->B < 2 || s->S <= ds::SMALL_MAX_S) return DS_OK;
+    const void *kern = cluster_kernel_of(s);
+    for (int cs = ds::CL_MAX_CS; cs >= 2; cs >>= 1) {
+        if ((long long)s->B * cs > s->num_sms || s->NQ / cs < ds::CL_CW) continue;
+        if (4LL * s->B * cs < 3LL * s->num_sms) break;
+        if (!cluster_layout(s, cs)) continue;
+        CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, ds::SMEM_MAX));
+        cudaLaunchConfig_t cfg;
+        memset(&cfg, 0, sizeof cfg);
+        cfg.gridDim = dim3((unsigned)cs, (unsigned)s->B); cfg.blockDim = dim3(ds::CL_NT); cfg.dynamicSmemBytes = s->cl_smem;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = (unsigned)cs; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        int n_active = 0;
+        CU_TRY(cudaOccupancyMaxActiveClusters(&n_active, kern, &cfg));
+        if (n_active >= s->B) { s->cl_cs = cs; return DS_OK; }
+    }
+    return DS_OK;
+}
+
+template <typename T, int TENSOR, bool HEUN>
+int launch_cluster_v(ds_system *s, const ds::ClusterArgs &A) {
+    auto kern = ds::cluster_kernel<T, TENSOR, HEUN>;
+    static SmemOptIn opt_in;
+    DS_TRY(opt_in.ensure((const void *)kern, s->P.device));
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof cfg);
+    cfg.gridDim = dim3((unsigned)A.cs, (unsigned)s->B); cfg.blockDim = dim3(ds::CL_NT);
+    cfg.dynamicSmemBytes = s->cl_smem; cfg.stream = s->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)A.cs; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    CU_TRY(cudaLaunchKernelEx(&cfg, kern, A));
+    s->launches += 1;
+    return DS_OK;
+}
+
+// RUN_STEP through the cluster kernel: one launch for all B systems
+int launch_cluster_run(ds_system *s, long long n_steps) {
+    ds::ClusterArgs A;
+    memset(&A, 0, sizeof A);
+    A.N = s->N; A.NQ = s->NQ; A.cs = s->cl_cs;
+    memcpy(A.half_off, s->cl_half_off, sizeof A.half_off);
+    A.buf_units[0] = s->cl_buf_units[0]; A.buf_units[1] = s->cl_buf_units[1];
+    A.rows_max = s->cl_rows_max; A.slots_max = s->cl_slots_max;
+    ds::RunArgs R;
+    memset(&R, 0, sizeof R);
+    fill_constants(s, R);
+    A.self_mob = R.self_mob; A.pre = R.pre; A.c1 = R.c1; A.c2 = R.c2; A.c1f = R.c1f; A.c2f = R.c2f;
+    A.t0 = R.t0; A.dt = R.dt; A.ell = R.ell; A.lambda = R.lambda; A.omega = R.omega; A.k0 = R.k0;
+    A.noise_amp = R.noise_amp; A.seed = R.seed;
+    A.n0 = s->n_host; A.n_steps = n_steps;
+    A.X = s->X; A.xu = s->xu; A.from_user = s->x_valid ? 0 : 1; A.phase = s->phase;
+    const bool heun = s->P.integrator == DS_HEUN, f64 = s->P.precision == DS_F64, rpy = s->P.tensor == DS_RPY;
+#define DS_CL(TT, TEN) (heun ? launch_cluster_v<TT, TEN, true>(s, A) : launch_cluster_v<TT, TEN, false>(s, A))
+    if (f64) DS_TRY(rpy ? DS_CL(double, ds::TENSOR_RPY) : DS_CL(double, ds::TENSOR_OSEEN));
+    else DS_TRY(rpy ? DS_CL(float, ds::TENSOR_RPY) : DS_CL(float, ds::TENSOR_OSEEN));
+#undef DS_CL
+    s->x_valid = true; s->xu_valid = true;
     return DS_OK;
 }
 
@@ -809,6 +928,7 @@ int ds_create(const ds_params *p, ds_system **out) {
     rc = choose_shape_step(s);   // N too large for one co-resident grid: the step modes cannot run
     if (rc != DS_OK) return fail(rc);
     rc = setup_pipe(s);
+    if (rc == DS_OK) rc = setup_cluster(s);
     if (rc != DS_OK) return fail(rc);
     const size_t n3 = (size_t)s->B * s->N * 3;
     const size_t ub = (size_t)s->B * (size_t)s->unit_stride * ds::UNIT_BYTES;
@@ -873,7 +993,8 @@ int ds_set_tuning(ds_system *s, int32_t n_tiles) {
     CU_TRY(cudaStreamSynchronize(s->stream));
     s->tune_cta = n_tiles;
     DS_TRY(choose_shape_step(s));
-    return setup_pipe(s);
+    DS_TRY(setup_pipe(s));
+    return setup_cluster(s);
 }
 
 int ds_set_pipeline(ds_system *s, int32_t mode) {
@@ -882,10 +1003,11 @@ int ds_set_pipeline(ds_system *s, int32_t mode) {
     DS_TRY(set_device(s));
     CU_TRY(cudaStreamSynchronize(s->stream));
     s->pipe_mode = mode;
-    return setup_pipe(s);
+    DS_TRY(setup_pipe(s));
+    return setup_cluster(s);
 }
 
-int ds_pipeline_active(const ds_system *s) { return s && s->use_pipe ? 1 : 0; }
+int ds_pipeline_active(const ds_system *s) { return !s ? 0 : (s->cl_cs > 0 ? 2 : (s->use_pipe ? 1 : 0)); }
 
 int ds_set_probe(ds_system *s, void *device_buffer) {
     if (!s) return DS_ERR_NULL;
@@ -1178,6 +1300,7 @@ int ds_batch_step(ds_system *s, int64_t n_steps) {
         const long long k = left < MAX_STEPS_PER_LAUNCH ? left : MAX_STEPS_PER_LAUNCH;
         // small systems: a warp per system; a forced tiling (ds_set_tuning) keeps them on run_kernel (tests)
         if (s->S <= ds::SMALL_MAX_S && s->tune_cta == 0) DS_TRY(launch_small_run(s, k));
+        else if (s->cl_cs > 0) DS_TRY(launch_cluster_run(s, k));
         else DS_TRY(s->use_pipe ? launch_pipe_run(s, k) : launch_state_run(s, ds::RUN_STEP, k, nullptr));
         s->n_host += k; left -= k;
     }

@@ -206,7 +206,7 @@ class System:
         _check(lib().ds_set_pipeline(self._h, int(mode)), "ds_set_pipeline")
 
     def pipeline_active(self):
-        return bool(lib().ds_pipeline_active(self._h))
+        return int(lib().ds_pipeline_active(self._h))   # 0 one-pass / warp-per-system, 1 pipelined, 2 cluster kernel
 
     def set_probe(self, buf=None):
         _check(lib().ds_set_probe(self._h, _ptr(buf)), "ds_set_probe")

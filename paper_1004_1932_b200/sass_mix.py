@@ -13,7 +13,7 @@ import sys
 from . import build
 
 OPS = ["FFMA2", "FMUL2", "FADD2", "FFMA", "DFMA", "DMUL", "DADD", "MUFU.RSQ", "MUFU.RSQ64H", "LDS", "UBLKCP", "LDGSTS", "SYNCS",
-       "USETMAXREG", "SHFL", "REDG", "BAR"]
+       "USETMAXREG", "SHFL", "REDG", "BAR", "STAS", "UCGABAR_ARV"]
 
 
 def demangle(names):
@@ -31,7 +31,7 @@ def main():
     rows = []
     for p in parts:
         name = p.split("\n", 1)[0].strip()
-        if "--all" not in sys.argv and not any(k in name for k in ("run_kernel", "pipe_kernel", "small_kernel", "avg_")):
+        if "--all" not in sys.argv and not any(k in name for k in ("run_kernel", "pipe_kernel", "cluster_kernel", "small_kernel", "apply_kernel", "avg_")):
             continue
         ins = re.findall(r"/\*[0-9a-f]{4,5}\*/\s+(?:@!?U?P\d\s+)?([A-Z0-9_.]+)([^;]*);", p)
         cnt = {o: 0 for o in OPS}

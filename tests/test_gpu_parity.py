@@ -864,3 +864,77 @@ def test_small_system_kernel_integrators_tensors_noise(integrator, tensor):
     for b in range(w.B):
         Xo = oracle.step(X0[b], w.phase[b], 0.25, 0, 101, dataclasses.replace(p, system=b))
         assert np.abs(Xa[b] - Xo).max() <= 1e-9 * ELL
+
+
+# --------------------------------------------------------------------------------- ensembles: one cluster per system (cluster.cuh)
+def cluster_steps(w, precision, chunks, tensor=ds.RPY, integrator=ds.HEUN, t0=0.0, host=False, expect=2, pipeline=-1, **kw):
+    """Steps of an ensemble through the library's own choice of kernel, which must be the cluster kernel (`expect` = 2;
+    `pipeline=0`, `expect=0` forces the one-pass kernel instead)."""
+    s, p = make_system(w, precision, tensor, integrator, **kw)
+    with s:
+        s.set_pipeline(pipeline)
+        assert s.pipeline_active() == expect, (w.B, w.S)
+        X0 = rounded(w, precision)
+        if host:
+            s.set_state(np.ascontiguousarray(X0, dtype=NPDT[precision]), np.ascontiguousarray(w.phase), t0=t0)
+        else:
+            s.set_state(dev(X0, precision), torch.as_tensor(w.phase, device="cuda"), t0=t0)
+        for c in chunks:
+            s.batch_step(c)
+        out = torch.empty((w.B, w.N, 3), dtype=TDT[precision], device="cuda")
+        s.get_state(out)
+        torch.cuda.synchronize()
+        return out.cpu().numpy().astype(np.float64), X0, p
+
+
+@pytest.mark.parametrize("precision,tol", [(ds.F32, 1e-4), (ds.F64, 1e-10)])
+@pytest.mark.parametrize("B,S,check", [(64, 256, (0, 17, 63)), (32, 256, (0, 31)), (74, 64, (0, 36, 73)), (70, 100, (0, 69)),
+                                       (70, 99, (0, 35, 69)), (14, 512, (3, 13)), (14, 700, (7,))])
+def test_cluster_kernel_shapes(B, S, check, precision, tol):
+    """Ensembles that get one thread-block cluster per system: 2 CTAs (B = 64, 74, 70), 4 (B = 32) and 8 (B = 14) per
+    system; halves of 32 quads (2 quads per warp, 16 lanes per quad), 16 (a warp per quad), 8 (2 warps per quad), 13 + 12
+    (idle warps), 22 + 22 and 22 + 21 (S = 700: idle warps and a warp whose second quad does not exist) and, with S = 99, a last quad of two rows; C5's own shape first.  Heun, t0 != 0, 9 steps over three calls,
+    against the oracle on a sample of the systems."""
+    w = inputs.config5(B=B, S=S)
+    Xg, X0, p = cluster_steps(w, precision, [4, 1, 4], t0=0.3)
+    for b in check:
+        Xo = oracle.step(X0[b], w.phase[b], 0.3, 0, 9, p)
+        assert np.abs(Xg[b] - Xo).max() <= tol * ELL, b
+
+
+@pytest.mark.parametrize("integrator", [ds.EULER, ds.HEUN])
+@pytest.mark.parametrize("tensor", [ds.OSEEN, ds.RPY])
+def test_cluster_kernel_integrators_tensors_chunking_determinism(integrator, tensor):
+    """Euler / Heun and both tensors through the cluster kernel (B = 32, S = 128: 4 CTAs per system); host buffers;
+    the result is bit-identical however the steps are split over launches and from run to run, and agrees with the one-pass
+    kernel to rounding."""
+    w = inputs.config5(B=32, S=128)
+    Xa, X0, p = cluster_steps(w, ds.F64, [31], tensor, integrator, t0=0.25)
+    Xb, _, _ = cluster_steps(w, ds.F64, [1, 13, 2, 15], tensor, integrator, t0=0.25, host=True)
+    assert np.array_equal(Xa, Xb)
+    Xc, _, _ = cluster_steps(w, ds.F64, [31], tensor, integrator, t0=0.25, pipeline=0, expect=0)
+    assert np.abs(Xa - Xc).max() <= 1e-10 * ELL
+    for b in (0, 31):
+        Xo = oracle.step(X0[b], w.phase[b], 0.25, 0, 31, p)
+        assert np.abs(Xa[b] - Xo).max() <= 1e-10 * ELL
+
+
+def test_cluster_kernel_with_additive_noise():
+    """k_B T > 0 through the cluster kernel: Philox increments drawn by the service warps, per system and sphere, steps
+    split over calls (B = 64, S = 64: 2 CTAs per system, FP64)."""
+    import dataclasses
+    w = inputs.config5(B=64, S=64)
+    Xg, X0, p = cluster_steps(w, ds.F64, [7, 13], kT=0.02, seed=0x1234567ABCDEF)
+    for b in (0, 40, 63):
+        Xo = oracle.step(X0[b], w.phase[b], 0.0, 0, 20, dataclasses.replace(p, system=b))
+        assert np.abs(Xg[b] - Xo).max() <= 1e-9 * ELL
+
+
+def test_cluster_kernel_not_taken_when_clusters_do_not_fit():
+    """Shapes the heuristic must leave to the other kernels: too few systems to fill 3/4 of the SMs (B = 48 x 2 CTAs),
+    more clusters than are resident at once (B = 37 x 4 CTAs in FP32), less than a quad per warp (S = 40), one system."""
+    for (B, S, precision) in ((48, 256, ds.F32), (37, 500, ds.F32), (64, 40, ds.F32), (1, 256, ds.F64)):
+        w = inputs.config5(B=B, S=S)
+        s, _ = make_system(w, precision)
+        with s:
+            assert s.pipeline_active() in (0, 1), (B, S)
