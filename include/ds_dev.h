@@ -36,7 +36,8 @@ int ds_peak_probe(int32_t precision, int32_t device, double *flops_per_s);
  * Ensembles (n_batch >= 2) whose systems can each take one thread-block cluster (cluster.cuh: all clusters resident at once
  * and filling at least 3/4 of the SMs) use the cluster kernel unless mode is 0.
  * ds_pipeline_active: the kernel the next ds_step / ds_batch_step would use: 0 = one-pass (or, for S <= 32, the
- * warp-per-system kernel), 1 = pipelined two-pass, 2 = cluster kernel.                                                   */
+ * warp-per-system kernel), 1 = pipelined two-pass, 2 = cluster kernel.
+ * Mode 2 (tests, measurements): the cluster kernel for every shape it can run, whatever the heuristic says.             */
 int ds_set_pipeline(ds_system *s, int32_t mode);
 int ds_pipeline_active(const ds_system *s);
 

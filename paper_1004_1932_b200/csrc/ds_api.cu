@@ -505,11 +505,13 @@ bool cluster_layout(ds_system *s, int cs) {
 // shared memory.
 int setup_cluster(ds_system *s) {
     s->cl_cs = 0;
-    if (s->pipe_mode == 0 || s->tune_cta != 0 || s->B < 2 || s->S <= ds::SMALL_MAX_S) return DS_OK;
+    const bool forced = s->pipe_mode == 2;   // ds_set_pipeline(2): whenever the layout fits and the clusters are co-resident
+    if (s->pipe_mode == 0 || s->tune_cta != 0 || ((s->B < 2 || s->S <= ds::SMALL_MAX_S) && !forced)) return DS_OK;
     const void *kern = cluster_kernel_of(s);
     for (int cs = ds::CL_MAX_CS; cs >= 2; cs >>= 1) {
-        if ((long long)s->B * cs > s->num_sms || s->NQ / cs < ds::CL_CW) continue;
-        if (4LL * s->B * cs < 3LL * s->num_sms) break;
+        if ((long long)s->B * cs > s->num_sms || cs > s->NQ) continue;
+        if (!forced && s->NQ / cs < ds::CL_CW) continue;
+        if (!forced && 4LL * s->B * cs < 3LL * s->num_sms) break;
         if (!cluster_layout(s, cs)) continue;
         CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, ds::SMEM_MAX));
         cudaLaunchConfig_t cfg;
@@ -576,6 +578,17 @@ template <typename T, int TENSOR, bool HEUN> int launch_small_v(ds_system *s, co
     CU_TRY(cudaGetLastError());
     s->launches += 1;
     return DS_OK;
+}
+
+// Warp-per-system kernel or run_kernel for S <= 32?  With 17 ... 32 dumbbells a lane has a whole dumbbell's pair sum to
+// itself (64 FP64 units at S = 32) and a stage takes 4.7 - 7.3 us in FP64 (2.4 - 3.6 in FP32) whatever B is; run_kernel on
+// several CTAs per system takes 3.2 - 3.5 us (2.8 - 3.0), but only as long as all systems are resident at once (measured,
+// B = 1 ... 600: DESIGN.md section 6c).  A forced tiling (ds_set_tuning) keeps small systems on run_kernel (tests).
+bool use_small_kernel(const ds_system *s) {
+    if (s->S > ds::SMALL_MAX_S || s->tune_cta != 0) return false;
+    if (s->S <= 16) return true;
+    if (s->P.precision == DS_F64) return (long long)s->B * s->n_cta > s->num_sms;
+    return s->S <= 24 || (long long)s->B * s->n_cta > s->num_sms;
 }
 
 int launch_small_run(ds_system *s, long long n_steps) {
@@ -999,7 +1012,7 @@ int ds_set_tuning(ds_system *s, int32_t n_tiles) {
 
 int ds_set_pipeline(ds_system *s, int32_t mode) {
     if (!s) return DS_ERR_NULL;
-    if (mode < -1 || mode > 1) return DS_ERR_INVALID_PARAM;
+    if (mode < -1 || mode > 2) return DS_ERR_INVALID_PARAM;
     DS_TRY(set_device(s));
     CU_TRY(cudaStreamSynchronize(s->stream));
     s->pipe_mode = mode;
@@ -1299,7 +1312,8 @@ int ds_batch_step(ds_system *s, int64_t n_steps) {
     while (left > 0) {   // one launch runs up to MAX_STEPS_PER_LAUNCH steps entirely on the device
         const long long k = left < MAX_STEPS_PER_LAUNCH ? left : MAX_STEPS_PER_LAUNCH;
         // small systems: a warp per system; a forced tiling (ds_set_tuning) keeps them on run_kernel (tests)
-        if (s->S <= ds::SMALL_MAX_S && s->tune_cta == 0) DS_TRY(launch_small_run(s, k));
+        if (s->cl_cs > 0 && s->pipe_mode == 2) DS_TRY(launch_cluster_run(s, k));
+        else if (use_small_kernel(s)) DS_TRY(launch_small_run(s, k));
         else if (s->cl_cs > 0) DS_TRY(launch_cluster_run(s, k));
         else DS_TRY(s->use_pipe ? launch_pipe_run(s, k) : launch_state_run(s, ds::RUN_STEP, k, nullptr));
         s->n_host += k; left -= k;

@@ -837,10 +837,11 @@ def test_step_state_in_global_memory_odd_S_batch():
 
 # --------------------------------------------------------------------------------- small systems: one warp per system (small.cuh)
 @pytest.mark.parametrize("precision,tol", [(ds.F32, 1e-4), (ds.F64, 1e-10)])
-@pytest.mark.parametrize("S,B", [(1, 1), (2, 3), (3, 1), (5, 7), (8, 1), (17, 5), (32, 9)])
+@pytest.mark.parametrize("S,B", [(1, 1), (2, 3), (3, 1), (5, 7), (8, 1), (17, 5), (32, 9), (17, 160), (32, 160)])
 def test_small_system_kernel_shapes(S, B, precision, tol):
     """S <= 32 dumbbells run one warp per system: 32, 16, 8, 4, 2, 1 lanes per dumbbell (S = 1 ... 32, powers of two and
-    not), several systems per CTA and a ragged last CTA.  60 Heun steps over three calls, t0 != 0, against the oracle;
+    not), several systems per CTA and a ragged last CTA; with 17 ... 32 dumbbells the warp-per-system kernel serves ensembles
+    too large to be resident on run_kernel at once (B = 160) and run_kernel the small ones.  60 Heun steps over three calls, t0 != 0, against the oracle;
     the same steps through run_kernel's one-CTA mode (forced tiling) agree to rounding."""
     w = inputs.config5(B=B, S=S)
     Xg, X0, p = gpu_steps(w, precision, 60, t0=0.1, chunks=[7, 1, 52])
