@@ -173,7 +173,7 @@ def time_steps(torch, ds, w, precision, tensor, n_steps, warmup, ranks=None, sam
         info = {"repeats": reps, "warmup_launches": wl, "warmup_device_ms": warm * 1e3,
                 "ms_per_step_min": 1e3 * t.min() / n_steps, "ms_per_step_max": 1e3 * t.max() / n_steps,
                 "timed_region_ms": 1e3 * t.sum(), "pipelined_kernel": s.pipeline_active() == 1,
-                "step_kernel": {0: "small" if w.S <= 32 else "one-pass", 1: "pipelined", 2: "cluster"}[s.pipeline_active()]}
+                "step_kernel": {0: "small" if w.S <= 16 else "one-pass", 1: "pipelined", 2: "cluster", 3: "cluster-latency"}[s.pipeline_active()]}
         return float(np.median(t)), int(launches), info
 
 

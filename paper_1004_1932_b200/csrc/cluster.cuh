@@ -400,4 +400,205 @@ __global__ void __launch_bounds__(CL_NT, 1) cluster_kernel(const ClusterArgs A) 
     cluster_barrier();   // nobody leaves while a peer could still address its shared memory
 }
 
+// ---------------------------------------------------------------------------------------------------------------------
+// The latency variant for single small systems and small ensembles (BASELINE.json config 2: N = 128): a stage there is not
+// arithmetic but the hand-over (3.1 us per stage on run_kernel's 32 CTAs through L2; 1.7 us of pair arithmetic alone on one
+// SM).  One cluster of cs = 8 CTAs per system, 512 threads, no service warps and no halves: every warp computes its place
+// of the pair sum over the whole stream (natural sphere order), the block finishes its rows (one thread per state
+// element, then one per dumbbell) and stores the dumbbells' units of the next stage into the shared memory of all CTAs
+// of the cluster with st.async onto the consumers' mbarriers, as above.  Two block barriers per stage, no cluster barrier.
+struct ClusterLatArgs {
+    int N, NQ, U, cs;
+    int buf_units;                // capacity of one stream buffer in units (U + pad, multiple of 8)
+    int rows_max, slots_max;
+    double self_mob, pre, c1, c2;
+    float c1f, c2f;
+    long long n0, n_steps;
+    double *X;
+    void *xu;
+    int from_user;
+    const double *phase;
+    double t0, dt, ell, lambda, omega, k0, noise_amp;
+    unsigned long long seed;
+};
+constexpr int CLL_NT = 512;
+
+template <typename T, int TENSOR, bool HEUN>
+__global__ void __launch_bounds__(CLL_NT, 1) cluster_lat_kernel(const ClusterLatArgs A) {
+    typedef Pack<T> P;
+    typedef typename P::V V;
+    constexpr int W = P::W;
+
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int r = blockIdx.x, b = blockIdx.y, cs = A.cs;
+    const size_t buf_bytes = (size_t)A.buf_units * UNIT_BYTES;
+    unsigned char *const after = smem_raw + 2 * buf_bytes;
+    uint64_t *const mb_full = reinterpret_cast<uint64_t *>(after);   // [parity]: the stage's stream has landed in this CTA
+    T *const scr = reinterpret_cast<T *>(after + 64);                // [slots_max][12]
+    double *const st = reinterpret_cast<double *>(after + 64 + (size_t)A.slots_max * 12 * 8);
+
+    const int q0 = (int)((long long)r * A.NQ / cs), q1 = (int)((long long)(r + 1) * A.NQ / cs);
+    const int nq = q1 - q0;
+    const long long r0 = 4LL * q0;
+    const int nrows = (int)((A.N - r0) < 4 * nq ? (A.N - r0) : 4 * nq);
+    const int nd = nrows >> 1;
+    const int rows_st = A.rows_max;
+    double *const Xs = st, *const Xc = st + 3 * rows_st, *const V1s = st + 6 * rows_st, *const Fs = st + 9 * rows_st;
+    double *const Ls = st + 12 * rows_st, *const phs = Ls + (rows_st >> 1);
+    T *const XcT = reinterpret_cast<T *>(st + 13 * rows_st);
+    const size_t sys3 = (size_t)b * A.N * 3;
+    const int n_stage = (int)(A.n_steps * (HEUN ? 2 : 1));
+    const uint32_t stream_bytes = (uint32_t)A.U * UNIT_BYTES;
+
+    // this warp's place (stage-invariant): quads per warp / warps per quad as in cluster_kernel, over nq quads
+    int QW, m;
+    cluster_pass_shape(nq, QW, m);
+    int lgG = 0;
+    while ((QW << lgG) < 32) ++lgG;
+    const int G = 1 << lgG, n_jg = G * m;
+    const int qfirst = (warp / m) * QW, sub = warp - (warp / m) * m;
+    const int quad = qfirst + (lane >> lgG), jg = (sub << lgG) + (lane & (G - 1));
+    const bool act = quad < nq, wact = qfirst < nq;
+    const int its = (A.U + n_jg - 1) / n_jg;
+    const int its_w = its - ((its > 0 && (its - 1) * n_jg + sub * G >= A.U) ? 1 : 0);
+    int g_lo = its_w, g_hi = its_w;
+    {   // iterations that may hold rows of this warp's quads (alpha == beta)
+        const int rl1 = 4 * (qfirst + QW) < nrows ? 4 * (qfirst + QW) : nrows;
+        const int uo0 = (int)((r0 + 4 * qfirst) / W), uo1 = (int)((r0 + rl1 + W - 1) / W);
+        if (wact && uo1 > uo0) {
+            g_lo = uo0 / n_jg; g_hi = (uo1 - 1) / n_jg + 1;
+            g_lo = g_lo < its_w ? g_lo : its_w; g_hi = g_hi < its_w ? g_hi : its_w;
+        }
+    }
+    const int slot = quad * m + sub, stride = 3 * n_jg;
+
+    auto publish_all = [&](int par, int sl, const double (&x0)[3], const double (&x1)[3], const double (&F0)[3]) {
+        const uint32_t dst = smem_u32(smem_raw + (size_t)par * buf_bytes) + (uint32_t)((r0 + 2 * sl) / W) * UNIT_BYTES;
+        const uint32_t bar = smem_u32(mb_full + par);
+        for (int p = 0; p < cs; ++p) publish_async(T(), mapa_u32(dst, (uint32_t)p), mapa_u32(bar, (uint32_t)p), x0, x1, F0);
+    };
+
+    // ---- prologue ----
+    for (int e = tid; e < 3 * nrows; e += CLL_NT) {
+        const double x = A.from_user ? (double)reinterpret_cast<const T *>(A.xu)[sys3 + 3 * r0 + e] : A.X[sys3 + 3 * r0 + e];
+        Xs[e] = x; Xc[e] = x; XcT[e] = (T)x;
+    }
+    for (int e = 3 * nrows + tid; e < 3 * rows_st; e += CLL_NT) XcT[e] = P::dummy();
+    for (int sl = tid; sl < nd; sl += CLL_NT) phs[sl] = A.phase[(size_t)b * (A.N / 2) + (r0 >> 1) + sl];
+    if (tid == 0) {
+        mbar_init(mb_full + 0, 1); mbar_init(mb_full + 1, 1);
+        mbar_fence_init();
+        mbar_expect_tx(mb_full + 0, stream_bytes); mbar_expect_tx(mb_full + 1, stream_bytes);
+    }
+    for (int k = 0; k < 2; ++k) {   // far-away zero-force pad units behind the stream (never overwritten)
+        uint4 *bp = reinterpret_cast<uint4 *>(smem_raw + (size_t)k * buf_bytes);
+        for (int j = 3 * A.U + tid; j < 3 * A.buf_units; j += CLL_NT) bp[j] = pad_piece<T>(j % 3);
+    }
+    cluster_barrier();
+    {
+        const double tn = time_of_step(A.t0, A.n0, A.dt);
+        for (int sl = tid; sl < nd; sl += CLL_NT) {
+            double x0[3], x1[3], F0[3];
+#pragma unroll
+            for (int cc = 0; cc < 3; ++cc) { x0[cc] = Xs[6 * sl + cc]; x1[cc] = Xs[6 * sl + 3 + cc]; }
+            dumbbell_force(x0, x1, stroke_length(tn, phs[sl], A.ell, A.lambda, A.omega), A.k0, F0);
+#pragma unroll
+            for (int cc = 0; cc < 3; ++cc) { Fs[6 * sl + cc] = F0[cc]; Fs[6 * sl + 3 + cc] = -F0[cc]; }
+            if (n_stage > 0) publish_all(0, sl, x0, x1, F0);
+        }
+    }
+    __syncthreads();
+
+    const V c1 = P::bc(sizeof(T) == 4 ? (T)A.c1f : (T)A.c1), negc2 = P::bc(sizeof(T) == 4 ? (T)(-A.c2f) : (T)(-A.c2));
+    for (int g = 0; g < n_stage; ++g) {
+        const int par = g & 1;
+        const bool pred = HEUN && (g & 1) == 0, corr = HEUN && (g & 1) == 1;
+        const long long nstep = A.n0 + (HEUN ? (g >> 1) : g);
+        // ---- pair sums ----
+        V xi[QI][3], acc[QI][3];
+#pragma unroll
+        for (int k = 0; k < QI; ++k) acc[k][0] = acc[k][1] = acc[k][2] = P::bc(T(0));
+        if (wact) {
+            T xq[12];
+            const typename P::T4 *xp = reinterpret_cast<const typename P::T4 *>(XcT + 12 * (act ? quad : qfirst));
+#pragma unroll
+            for (int k = 0; k < 3; ++k) { const typename P::T4 q = xp[k]; xq[4 * k] = q.x; xq[4 * k + 1] = q.y; xq[4 * k + 2] = q.z; xq[4 * k + 3] = q.w; }
+#pragma unroll
+            for (int k = 0; k < QI; ++k) { xi[k][0] = P::bc(xq[3 * k]); xi[k][1] = P::bc(xq[3 * k + 1]); xi[k][2] = P::bc(xq[3 * k + 2]); }
+        }
+        mbar_wait_cluster(mb_full + par, (uint32_t)(g >> 1) & 1u);
+        if (act) {
+            const V2<T> *p = reinterpret_cast<const V2<T> *>(smem_raw + (size_t)par * buf_bytes) + 3 * jg;
+            int it = 0;
+#pragma unroll 1
+            for (; it < g_lo; ++it, p += stride) pair_unit<T, TENSOR, false>(p, xi, acc, c1, negc2);
+#pragma unroll 1
+            for (; it < g_hi; ++it, p += stride) pair_unit<T, TENSOR, true>(p, xi, acc, c1, negc2);
+#pragma unroll 1
+            for (; it < its_w; ++it, p += stride) pair_unit<T, TENSOR, false>(p, xi, acc, c1, negc2);
+        }
+        if (wact) {
+            T v[12], s3[3];
+#pragma unroll
+            for (int k = 0; k < QI; ++k)
+#pragma unroll
+                for (int cc = 0; cc < 3; ++cc) v[3 * k + cc] = P::hsum(acc[k][cc]);
+            group_sum12<T>(v, lane, G, s3);
+            if (act && (lane & ((G >> 2) - 1)) == 0) {
+                const int j = ((lane & (G >> 1)) ? 2 : 0) + ((lane & (G >> 2)) ? 1 : 0);
+                T *dst = scr + (size_t)slot * 12 + 3 * j;
+                dst[0] = s3[0]; dst[1] = s3[1]; dst[2] = s3[2];
+            }
+        }
+        __syncthreads();
+        // ---- tail, part 1: one thread per own state element; spare threads take the stroke lengths of the next step ----
+        const bool last = g + 1 == n_stage;
+        const double cdt = corr ? 0.5 * A.dt : A.dt;
+        const int n_item = 3 * nrows + ((!HEUN || (g & 1) == 0) ? nd : 0);
+        for (int i = tid; i < n_item; i += CLL_NT) {
+            if (i >= 3 * nrows) {   // L(t_{n+1}), once per step
+                const int sl = i - 3 * nrows;
+                Ls[sl] = stroke_length(time_of_step(A.t0, nstep + 1, A.dt), phs[sl], A.ell, A.lambda, A.omega);
+                continue;
+            }
+            const int E = i, rl = E / 3, cc = E - 3 * rl, qd = rl >> 2, k = rl & 3;
+            const T *sp = scr + (size_t)(qd * m) * 12 + 3 * k + cc;
+            T sacc = T(0);                                  // the m warps of the quad, in order
+#pragma unroll 1
+            for (int j = 0; j < m; ++j) sacc += sp[12 * j];
+            // Eq. (3a), the 1/(8 pi mu) factor and the integrator in FP64
+            const double v = A.self_mob * Fs[E] + A.pre * (double)sacc;
+            const double w = corr ? V1s[E] + v : v;
+            double xn = Xs[E] + cdt * w;
+            if (A.noise_amp != 0.0) xn += A.noise_amp * noise_normal(A.seed, nstep, b, 3 * r0 + E);
+            if (pred) V1s[E] = v; else Xs[E] = xn;
+            Xc[E] = xn;
+            XcT[E] = (T)xn;
+        }
+        // every warp of this CTA has passed stage g's wait: arm the barrier for stage g + 2 (no peer can send that stream
+        // before it has received this CTA's rows of stage g + 1, which leave after the next block barrier)
+        if (tid == 0 && g + 2 < n_stage) mbar_expect_tx(mb_full + par, stream_bytes);
+        __syncthreads();
+        // ---- tail, part 2: Eq. (4) at the new positions and time; the dumbbell's unit of the next stage, into every CTA ----
+        for (int sl = tid; sl < nd; sl += CLL_NT) {
+            double x0[3], x1[3], F0[3];
+#pragma unroll
+            for (int cc = 0; cc < 3; ++cc) { x0[cc] = Xc[6 * sl + cc]; x1[cc] = Xc[6 * sl + 3 + cc]; }
+            dumbbell_force(x0, x1, Ls[sl], A.k0, F0);
+#pragma unroll
+            for (int cc = 0; cc < 3; ++cc) { Fs[6 * sl + cc] = F0[cc]; Fs[6 * sl + 3 + cc] = -F0[cc]; }
+            if (!last) publish_all((g + 1) & 1, sl, x0, x1, F0);
+        }
+        // Fs of this stage is read by part 1 of the next stage, behind that stage's first block barrier
+    }
+    __syncthreads();
+    for (int e = tid; e < 3 * nrows; e += CLL_NT) {
+        const double x = Xs[e];
+        A.X[sys3 + 3 * r0 + e] = x;
+        reinterpret_cast<T *>(A.xu)[sys3 + 3 * r0 + e] = (T)x;
+    }
+    cluster_barrier();   // nobody leaves while a peer could still address its shared memory
+}
+
 }  // namespace ds

@@ -105,6 +105,8 @@ struct ds_system {
     int cl_cs = 0;                              // > 0: cluster_kernel with this many CTAs per system (cluster.cuh)
     int cl_buf_units[2] = {0, 0}, cl_rows_max = 0, cl_slots_max = 0;
     int cl_half_off[2][ds::CL_MAX_CS + 1] = {};
+    int cll_cs = 0, cll_buf_units = 0, cll_rows_max = 0, cll_slots_max = 0;   // > 0: cluster_lat_kernel (cluster.cuh)
+    size_t cll_smem = 0;
     size_t cl_smem = 0;
     int *half_off = nullptr;                    // device table [2][n_cta + 1]
     int half_off_cap = 0;
@@ -612,6 +614,100 @@ int launch_small_run(ds_system *s, long long n_steps) {
     return DS_OK;
 }
 
+// the latency variant of the cluster kernel a system uses
+const void *cluster_lat_kernel_of(const ds_system *s) {
+    const bool heun = s->P.integrator == DS_HEUN, f64 = s->P.precision == DS_F64, rpy = s->P.tensor == DS_RPY;
+#define DS_CLK(TT, TEN) (heun ? (const void *)ds::cluster_lat_kernel<TT, TEN, true> : (const void *)ds::cluster_lat_kernel<TT, TEN, false>)
+    if (f64) return rpy ? DS_CLK(double, ds::TENSOR_RPY) : DS_CLK(double, ds::TENSOR_OSEEN);
+    return rpy ? DS_CLK(float, ds::TENSOR_RPY) : DS_CLK(float, ds::TENSOR_OSEEN);
+#undef DS_CLK
+}
+
+// cluster_lat_kernel (cluster.cuh) for single small systems and small ensembles: one cluster of 8 (4, 2) CTAs per system when
+// all B clusters are resident at once and a stage's pair loops are short (at most LAT_MAX_ITERS iterations per warp: beyond
+// that the 148-SM shapes of run_kernel / pipe_kernel win).  ds_set_pipeline(3) forces it for every shape that fits.
+// Measured (FP32 / FP64 us per stage, this kernel against the earlier choice): S = 20: 1.9 / 2.3 against 2.5 / 3.3; S = 64
+// (C2): 1.9 / 2.3 against 3.1 / 3.5; S = 128: 2.4 / 4.0 against 3.2 / 4.1; S = 192: 3.6 / 6.9 against 3.7 / 4.7; 18 x S = 64:
+// 1.8 / 2.8 against 3.2 / 5.2.  S <= 16 stays on the warp-per-system kernel (0.8 - 2.2 us).
+constexpr int LAT_MAX_ITERS_F32 = 4, LAT_MAX_ITERS_F64 = 3;
+int setup_cluster_lat(ds_system *s) {
+    s->cll_cs = 0;
+    const bool forced = s->pipe_mode == 3;
+    const int LAT_MAX_ITERS = s->P.precision == DS_F64 ? LAT_MAX_ITERS_F64 : LAT_MAX_ITERS_F32;
+    if (s->pipe_mode == 0 || s->pipe_mode == 2 || s->tune_cta != 0 || s->cl_cs > 0) return DS_OK;
+    if (!forced && (s->pipe_mode == 1 || s->S <= 16)) return DS_OK;
+    const void *kern = cluster_lat_kernel_of(s);
+    for (int cs = ds::CL_MAX_CS; cs >= 2; cs >>= 1) {
+        if ((long long)s->B * cs > s->num_sms || cs > s->NQ) continue;
+        const int nq = (s->NQ + cs - 1) / cs;
+        if (nq > ds::CL_CW * ds::CL_MAX_QW) continue;
+        int njg = 32, slots = 1, its = 0;
+        for (int n = s->NQ / cs; n <= nq; ++n) {   // CTAs own floor or ceil(NQ / cs) quads
+            int QW, m;
+            ds::cluster_pass_shape(n, QW, m);
+            const int j = (32 / QW) * m, i = (s->U + j - 1) / j;
+            njg = njg > j ? njg : j; slots = slots > n * m ? slots : n * m; its = its > i ? its : i;
+        }
+        if (!forced && its > LAT_MAX_ITERS) continue;
+        const int buf_units = (s->U + njg + 7) / 8 * 8, rows_max = 4 * nq;
+        const size_t smem = 2 * (size_t)buf_units * ds::UNIT_BYTES + 64 + (size_t)slots * 12 * 8 + (size_t)rows_max * ds::STATE_BYTES_PER_ROW;
+        if (smem > (size_t)ds::SMEM_MAX) continue;
+        CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, ds::SMEM_MAX));
+        cudaLaunchConfig_t cfg;
+        memset(&cfg, 0, sizeof cfg);
+        cfg.gridDim = dim3((unsigned)cs, (unsigned)s->B); cfg.blockDim = dim3(ds::CLL_NT); cfg.dynamicSmemBytes = smem;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = (unsigned)cs; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        int n_active = 0;
+        CU_TRY(cudaOccupancyMaxActiveClusters(&n_active, kern, &cfg));
+        if (n_active < s->B) continue;
+        s->cll_cs = cs; s->cll_buf_units = buf_units; s->cll_rows_max = rows_max; s->cll_slots_max = slots; s->cll_smem = smem;
+        return DS_OK;
+    }
+    return DS_OK;
+}
+
+template <typename T, int TENSOR, bool HEUN>
+int launch_cluster_lat_v(ds_system *s, const ds::ClusterLatArgs &A) {
+    auto kern = ds::cluster_lat_kernel<T, TENSOR, HEUN>;
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof cfg);
+    cfg.gridDim = dim3((unsigned)A.cs, (unsigned)s->B); cfg.blockDim = dim3(ds::CLL_NT);
+    cfg.dynamicSmemBytes = s->cll_smem; cfg.stream = s->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)A.cs; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    CU_TRY(cudaLaunchKernelEx(&cfg, kern, A));
+    s->launches += 1;
+    return DS_OK;
+}
+
+int launch_cluster_lat_run(ds_system *s, long long n_steps) {
+    ds::ClusterLatArgs A;
+    memset(&A, 0, sizeof A);
+    A.N = s->N; A.NQ = s->NQ; A.U = s->U; A.cs = s->cll_cs;
+    A.buf_units = s->cll_buf_units; A.rows_max = s->cll_rows_max; A.slots_max = s->cll_slots_max;
+    ds::RunArgs R;
+    memset(&R, 0, sizeof R);
+    fill_constants(s, R);
+    A.self_mob = R.self_mob; A.pre = R.pre; A.c1 = R.c1; A.c2 = R.c2; A.c1f = R.c1f; A.c2f = R.c2f;
+    A.t0 = R.t0; A.dt = R.dt; A.ell = R.ell; A.lambda = R.lambda; A.omega = R.omega; A.k0 = R.k0;
+    A.noise_amp = R.noise_amp; A.seed = R.seed;
+    A.n0 = s->n_host; A.n_steps = n_steps;
+    A.X = s->X; A.xu = s->xu; A.from_user = s->x_valid ? 0 : 1; A.phase = s->phase;
+    const bool heun = s->P.integrator == DS_HEUN, f64 = s->P.precision == DS_F64, rpy = s->P.tensor == DS_RPY;
+#define DS_CL(TT, TEN) (heun ? launch_cluster_lat_v<TT, TEN, true>(s, A) : launch_cluster_lat_v<TT, TEN, false>(s, A))
+    if (f64) DS_TRY(rpy ? DS_CL(double, ds::TENSOR_RPY) : DS_CL(double, ds::TENSOR_OSEEN));
+    else DS_TRY(rpy ? DS_CL(float, ds::TENSOR_RPY) : DS_CL(float, ds::TENSOR_OSEEN));
+#undef DS_CL
+    s->x_valid = true; s->xu_valid = true;
+    return DS_OK;
+}
+
+
 // RUN_VELOCITY (n_steps ignored) or RUN_STEP on the system's own state: one launch per group of
 // co-resident systems; the barrier counters advance by n_cta per stage.
 int launch_state_run(ds_system *s, int mode, long long n_steps, void *out_u) {
@@ -942,6 +1038,7 @@ int ds_create(const ds_params *p, ds_system **out) {
     if (rc != DS_OK) return fail(rc);
     rc = setup_pipe(s);
     if (rc == DS_OK) rc = setup_cluster(s);
+    if (rc == DS_OK) rc = setup_cluster_lat(s);
     if (rc != DS_OK) return fail(rc);
     const size_t n3 = (size_t)s->B * s->N * 3;
     const size_t ub = (size_t)s->B * (size_t)s->unit_stride * ds::UNIT_BYTES;
@@ -1007,20 +1104,22 @@ int ds_set_tuning(ds_system *s, int32_t n_tiles) {
     s->tune_cta = n_tiles;
     DS_TRY(choose_shape_step(s));
     DS_TRY(setup_pipe(s));
-    return setup_cluster(s);
+    DS_TRY(setup_cluster(s));
+    return setup_cluster_lat(s);
 }
 
 int ds_set_pipeline(ds_system *s, int32_t mode) {
     if (!s) return DS_ERR_NULL;
-    if (mode < -1 || mode > 2) return DS_ERR_INVALID_PARAM;
+    if (mode < -1 || mode > 3) return DS_ERR_INVALID_PARAM;
     DS_TRY(set_device(s));
     CU_TRY(cudaStreamSynchronize(s->stream));
     s->pipe_mode = mode;
     DS_TRY(setup_pipe(s));
-    return setup_cluster(s);
+    DS_TRY(setup_cluster(s));
+    return setup_cluster_lat(s);
 }
 
-int ds_pipeline_active(const ds_system *s) { return !s ? 0 : (s->cl_cs > 0 ? 2 : (s->use_pipe ? 1 : 0)); }
+int ds_pipeline_active(const ds_system *s) { return !s ? 0 : (s->cl_cs > 0 ? 2 : (s->cll_cs > 0 ? 3 : (s->use_pipe ? 1 : 0))); }
 
 int ds_set_probe(ds_system *s, void *device_buffer) {
     if (!s) return DS_ERR_NULL;
@@ -1313,6 +1412,7 @@ int ds_batch_step(ds_system *s, int64_t n_steps) {
         const long long k = left < MAX_STEPS_PER_LAUNCH ? left : MAX_STEPS_PER_LAUNCH;
         // small systems: a warp per system; a forced tiling (ds_set_tuning) keeps them on run_kernel (tests)
         if (s->cl_cs > 0 && s->pipe_mode == 2) DS_TRY(launch_cluster_run(s, k));
+        else if (s->cll_cs > 0) DS_TRY(launch_cluster_lat_run(s, k));
         else if (use_small_kernel(s)) DS_TRY(launch_small_run(s, k));
         else if (s->cl_cs > 0) DS_TRY(launch_cluster_run(s, k));
         else DS_TRY(s->use_pipe ? launch_pipe_run(s, k) : launch_state_run(s, ds::RUN_STEP, k, nullptr));

@@ -31,7 +31,7 @@ def main():
     rows = []
     for p in parts:
         name = p.split("\n", 1)[0].strip()
-        if "--all" not in sys.argv and not any(k in name for k in ("run_kernel", "pipe_kernel", "cluster_kernel", "small_kernel", "apply_kernel", "avg_")):
+        if "--all" not in sys.argv and not any(k in name for k in ("run_kernel", "pipe_kernel", "cluster_kernel", "cluster_lat_kernel", "small_kernel", "apply_kernel", "avg_")):
             continue
         ins = re.findall(r"/\*[0-9a-f]{4,5}\*/\s+(?:@!?U?P\d\s+)?([A-Z0-9_.]+)([^;]*);", p)
         cnt = {o: 0 for o in OPS}

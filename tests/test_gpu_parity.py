@@ -938,4 +938,55 @@ def test_cluster_kernel_not_taken_when_clusters_do_not_fit():
         w = inputs.config5(B=B, S=S)
         s, _ = make_system(w, precision)
         with s:
-            assert s.pipeline_active() in (0, 1), (B, S)
+            assert s.pipeline_active() in (0, 1, 3), (B, S)   # 3: the latency variant (short pair loops), tested below
+
+
+# --------------------------------------------------------------------------------- small systems: a cluster of CTAs, no pipeline (cluster_lat_kernel)
+@pytest.mark.parametrize("precision,tol", [(ds.F32, 1e-4), (ds.F64, 1e-10)])
+@pytest.mark.parametrize("B,S", [(1, 17), (1, 33), (3, 40), (1, 64), (2, 99), (1, 128), (18, 64), (64, 40), (37, 64)])
+def test_cluster_lat_kernel_shapes(B, S, precision, tol):
+    """Systems with short pair loops on one cluster each (cluster_lat_kernel): 8 CTAs per system with 1 - 8 quads per CTA
+    (16 ... 2 warps per quad; S = 17, 33: CTAs of 1 and 2 / 2 and 3 quads, S = 99: a last quad of two rows), 2 CTAs per
+    system in ensembles of 64 and 37 (a warp per quad, idle warps); C2's shape (S = 64).  40 Heun steps over three calls,
+    t0 != 0, against the oracle on every system (a sample for the big ensembles)."""
+    w = inputs.config5(B=B, S=S)
+    Xg, X0, p = cluster_steps(w, precision, [7, 1, 32], t0=0.1, expect=3, pipeline=3)   # forced: the heuristic is tested below
+    for b in sorted({0, B // 2, B - 1}):
+        Xo = oracle.step(X0[b], w.phase[b], 0.1, 0, 40, p)
+        assert np.abs(Xg[b] - Xo).max() <= tol * ELL, b
+
+
+@pytest.mark.parametrize("integrator", [ds.EULER, ds.HEUN])
+@pytest.mark.parametrize("tensor", [ds.OSEEN, ds.RPY])
+def test_cluster_lat_kernel_integrators_tensors_noise_chunking(integrator, tensor):
+    """Euler / Heun, Oseen / RPY, k_B T > 0 through cluster_lat_kernel (C2's lattice, B = 1 and an ensemble of 5): bit-identical
+    however the steps are split over launches, from host buffers too; against the oracle; forced on a shape the heuristic
+    leaves to run_kernel (S = 300: 10 iterations per warp) it still agrees."""
+    import dataclasses
+    w = inputs.config2()
+    Xa, X0, p = cluster_steps(w, ds.F64, [101], tensor, integrator, t0=0.25, expect=3, kT=0.02, seed=0xABCDEF12345)
+    Xb, _, _ = cluster_steps(w, ds.F64, [1, 33, 3, 64], tensor, integrator, t0=0.25, expect=3, host=True, kT=0.02, seed=0xABCDEF12345)
+    assert np.array_equal(Xa, Xb)
+    Xo = oracle.step(X0[0], w.phase[0], 0.25, 0, 101, p)
+    assert np.abs(Xa[0] - Xo).max() <= 1e-9 * ELL
+    w5 = inputs.config5(B=5, S=48)
+    Xc, X05, p5 = cluster_steps(w5, ds.F32, [20, 21], tensor, integrator, expect=3, kT=0.01, seed=77)
+    for b in range(w5.B):
+        Xo = oracle.step(X05[b], w5.phase[b], 0.0, 0, 41, dataclasses.replace(p5, system=b))
+        assert np.abs(Xc[b] - Xo).max() <= 1e-4 * ELL
+    w3 = inputs.config5(B=2, S=300)
+    Xd, X03, p3 = cluster_steps(w3, ds.F64, [9], tensor, integrator, expect=3, pipeline=3)
+    for b in range(w3.B):
+        Xo = oracle.step(X03[b], w3.phase[b], 0.0, 0, 9, p3)
+        assert np.abs(Xd[b] - Xo).max() <= 1e-10 * ELL
+
+
+def test_cluster_lat_kernel_heuristic():
+    """Which shapes the library sends to cluster_lat_kernel by itself: short pair loops only (C2 yes, S = 300 no), never S <= 16
+    (warp-per-system kernel), never when the clusters are not resident at once (B = 100 x 2 CTAs)."""
+    for (B, S, precision, want) in ((1, 64, ds.F32, 3), (1, 64, ds.F64, 3), (18, 64, ds.F32, 3), (1, 20, ds.F64, 3), (1, 8, ds.F64, 0),
+                                    (1, 16, ds.F32, 0), (1, 300, ds.F64, 0), (100, 33, ds.F32, 0), (64, 256, ds.F32, 2)):
+        w = inputs.config5(B=B, S=S)
+        s, _ = make_system(w, precision)
+        with s:
+            assert s.pipeline_active() == want, (B, S, precision)
