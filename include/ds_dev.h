@@ -35,8 +35,8 @@ int ds_peak_probe(int32_t precision, int32_t device, double *flops_per_s);
  * equations; they differ in the order of the split-beta sums, i.e. in the last bits.
  * Ensembles (n_batch >= 2) whose systems can each take one thread-block cluster (cluster.cuh: all clusters resident at once
  * and filling at least 3/4 of the SMs) use the cluster kernel unless mode is 0.
- * Systems with short pair loops (17 <= S up to about 130 in FP32; at most 4 / 3 iterations per warp in FP32 / FP64) whose
- * clusters of 8, 4 or 2 CTAs are all resident at once use the latency variant cluster_lat_kernel unless mode is 0 or 1.
+ * Systems with short pair loops (17 <= S up to about 200 in FP32, 130 in FP64: at most 3 iterations per warp, 4 in ensembles)
+ * whose clusters of 2 ... 16 CTAs are all resident at once use the latency variant cluster_lat_kernel unless mode is 0 or 1.
  * ds_pipeline_active: the kernel the next ds_step / ds_batch_step would use: 0 = one-pass (or, for small S, the
  * warp-per-system kernel), 1 = pipelined two-pass, 2 = cluster kernel, 3 = its latency variant.
  * Modes 2 and 3 (tests, measurements): the cluster kernel / its latency variant for every shape they can run, whatever the

@@ -34,7 +34,7 @@ namespace ds {
 
 constexpr int CL_CW = 16;                        // compute warps
 constexpr int CL_NT = 32 * (CL_CW + 4);          // + the service warpgroup
-constexpr int CL_MAX_CS = 8;                     // portable cluster size
+constexpr int CL_MAX_CS = 8;                     // portable cluster size (the latency variant also takes 16)
 constexpr int CL_MAX_QW = 8;                     // quads per warp (lanes per quad >= 4)
 constexpr int CL_BAR_BYTES = 128;                // 8 mbarriers
 constexpr int CL_TAB_BYTES = 2 * CL_CW * 2 * 16; // per pass and warp: its place and loop bounds (stage-invariant)

@@ -623,21 +623,26 @@ const void *cluster_lat_kernel_of(const ds_system *s) {
 #undef DS_CLK
 }
 
-// cluster_lat_kernel (cluster.cuh) for single small systems and small ensembles: one cluster of 8 (4, 2) CTAs per system when
+// cluster_lat_kernel (cluster.cuh) for single small systems and small ensembles: one cluster of 2 ... 16 CTAs per system when
 // all B clusters are resident at once and a stage's pair loops are short (at most LAT_MAX_ITERS iterations per warp: beyond
 // that the 148-SM shapes of run_kernel / pipe_kernel win).  ds_set_pipeline(3) forces it for every shape that fits.
-// Measured (FP32 / FP64 us per stage, this kernel against the earlier choice): S = 20: 1.9 / 2.3 against 2.5 / 3.3; S = 64
-// (C2): 1.9 / 2.3 against 3.1 / 3.5; S = 128: 2.4 / 4.0 against 3.2 / 4.1; S = 192: 3.6 / 6.9 against 3.7 / 4.7; 18 x S = 64:
+// Measured (FP32 / FP64 us per stage, this kernel against the earlier choice): S = 20: 1.6 / 2.0 against 2.5 / 3.3; S = 64
+// (C2): 1.8 / 2.3 against 3.1 / 3.5; S = 128: 2.2 / 3.3 against 3.2 / 4.1; S = 192: 2.7 / 4.7 against 3.7 / 4.7; 18 x S = 64:
 // 1.8 / 2.8 against 3.2 / 5.2.  S <= 16 stays on the warp-per-system kernel (0.8 - 2.2 us).
-constexpr int LAT_MAX_ITERS_F32 = 4, LAT_MAX_ITERS_F64 = 3;
+// ... and, at 4 iterations per warp: single systems S = 256 FP32 3.7 against 3.6, S = 160 FP64 4.1 against 4.3 (a tie), but ensembles
+// 18 x S = 128 FP32 3.3 against 4.4, 16 x S = 128 FP64 6.1 against 7.1 (run_kernel has fewer CTAs per system there).
+constexpr int LAT_MAX_ITERS_SINGLE = 3, LAT_MAX_ITERS_ENSEMBLE = 4;
 int setup_cluster_lat(ds_system *s) {
     s->cll_cs = 0;
     const bool forced = s->pipe_mode == 3;
-    const int LAT_MAX_ITERS = s->P.precision == DS_F64 ? LAT_MAX_ITERS_F64 : LAT_MAX_ITERS_F32;
+    const int LAT_MAX_ITERS = s->B >= 2 ? LAT_MAX_ITERS_ENSEMBLE : LAT_MAX_ITERS_SINGLE;
     if (s->pipe_mode == 0 || s->pipe_mode == 2 || s->tune_cta != 0 || s->cl_cs > 0) return DS_OK;
     if (!forced && (s->pipe_mode == 1 || s->S <= 16)) return DS_OK;
     const void *kern = cluster_lat_kernel_of(s);
-    for (int cs = ds::CL_MAX_CS; cs >= 2; cs >>= 1) {
+    int best_its = 1 << 30;
+    // 16 CTAs per cluster is beyond the portable size (opt-in attribute); the smallest cluster with the fewest iterations wins
+    // (S = 64: 8 CTAs 1.9 us per stage, 16 CTAs 2.0; S = 128: 2.4 / 2.2; S = 192: 3.6 / 2.7)
+    for (int cs = 2; cs <= 16; cs <<= 1) {
         if ((long long)s->B * cs > s->num_sms || cs > s->NQ) continue;
         const int nq = (s->NQ + cs - 1) / cs;
         if (nq > ds::CL_CW * ds::CL_MAX_QW) continue;
@@ -648,11 +653,15 @@ int setup_cluster_lat(ds_system *s) {
             const int j = (32 / QW) * m, i = (s->U + j - 1) / j;
             njg = njg > j ? njg : j; slots = slots > n * m ? slots : n * m; its = its > i ? its : i;
         }
-        if (!forced && its > LAT_MAX_ITERS) continue;
+        if (its >= best_its || (!forced && its > LAT_MAX_ITERS)) continue;
         const int buf_units = (s->U + njg + 7) / 8 * 8, rows_max = 4 * nq;
         const size_t smem = 2 * (size_t)buf_units * ds::UNIT_BYTES + 64 + (size_t)slots * 12 * 8 + (size_t)rows_max * ds::STATE_BYTES_PER_ROW;
         if (smem > (size_t)ds::SMEM_MAX) continue;
         CU_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, ds::SMEM_MAX));
+        if (cs > ds::CL_MAX_CS && cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) {
+            (void)cudaGetLastError();
+            continue;
+        }
         cudaLaunchConfig_t cfg;
         memset(&cfg, 0, sizeof cfg);
         cfg.gridDim = dim3((unsigned)cs, (unsigned)s->B); cfg.blockDim = dim3(ds::CLL_NT); cfg.dynamicSmemBytes = smem;
@@ -661,10 +670,10 @@ int setup_cluster_lat(ds_system *s) {
         at[0].val.clusterDim.x = (unsigned)cs; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
         cfg.attrs = at; cfg.numAttrs = 1;
         int n_active = 0;
-        CU_TRY(cudaOccupancyMaxActiveClusters(&n_active, kern, &cfg));
+        if (cudaOccupancyMaxActiveClusters(&n_active, kern, &cfg) != cudaSuccess) { (void)cudaGetLastError(); continue; }
         if (n_active < s->B) continue;
+        best_its = its;
         s->cll_cs = cs; s->cll_buf_units = buf_units; s->cll_rows_max = rows_max; s->cll_slots_max = slots; s->cll_smem = smem;
-        return DS_OK;
     }
     return DS_OK;
 }

@@ -946,7 +946,7 @@ def test_cluster_kernel_not_taken_when_clusters_do_not_fit():
 @pytest.mark.parametrize("B,S", [(1, 17), (1, 33), (3, 40), (1, 64), (2, 99), (1, 128), (18, 64), (64, 40), (37, 64)])
 def test_cluster_lat_kernel_shapes(B, S, precision, tol):
     """Systems with short pair loops on one cluster each (cluster_lat_kernel): 8 CTAs per system with 1 - 8 quads per CTA
-    (16 ... 2 warps per quad; S = 17, 33: CTAs of 1 and 2 / 2 and 3 quads, S = 99: a last quad of two rows), 2 CTAs per
+    (16 ... 2 warps per quad; S = 17, 33: CTAs of uneven quad counts, S = 99: a last quad of two rows), 2 CTAs per
     system in ensembles of 64 and 37 (a warp per quad, idle warps); C2's shape (S = 64).  40 Heun steps over three calls,
     t0 != 0, against the oracle on every system (a sample for the big ensembles)."""
     w = inputs.config5(B=B, S=S)
