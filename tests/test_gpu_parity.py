@@ -943,12 +943,12 @@ def test_cluster_kernel_not_taken_when_clusters_do_not_fit():
 
 # --------------------------------------------------------------------------------- small systems: a cluster of CTAs, no pipeline (cluster_lat_kernel)
 @pytest.mark.parametrize("precision,tol", [(ds.F32, 1e-4), (ds.F64, 1e-10)])
-@pytest.mark.parametrize("B,S", [(1, 17), (1, 33), (3, 40), (1, 64), (2, 99), (1, 128), (18, 64), (64, 40), (37, 64)])
+@pytest.mark.parametrize("B,S", [(1, 17), (1, 33), (3, 40), (1, 64), (2, 99), (1, 128), (12, 128), (18, 64), (64, 40), (37, 64)])
 def test_cluster_lat_kernel_shapes(B, S, precision, tol):
-    """Systems with short pair loops on one cluster each (cluster_lat_kernel): 8 CTAs per system with 1 - 8 quads per CTA
-    (16 ... 2 warps per quad; S = 17, 33: CTAs of uneven quad counts, S = 99: a last quad of two rows), 2 CTAs per
-    system in ensembles of 64 and 37 (a warp per quad, idle warps); C2's shape (S = 64).  40 Heun steps over three calls,
-    t0 != 0, against the oracle on every system (a sample for the big ensembles)."""
+    """Systems with short pair loops on one cluster each (cluster_lat_kernel), the cluster size the library picks: 2 CTAs per
+    system (S = 17; the ensembles of 64 and 37), 4 (S = 33, 40, 64 = C2's shape; 18 x S = 64), 8 (12 x S = 128), 16 (S = 99, 128);
+    1 - 16 quads per CTA (16 ... 1 warps per quad, idle warps, CTAs of uneven quad counts; S = 99: a last quad of two rows).
+    40 Heun steps over three calls, t0 != 0, against the oracle on every system (a sample for the big ensembles)."""
     w = inputs.config5(B=B, S=S)
     Xg, X0, p = cluster_steps(w, precision, [7, 1, 32], t0=0.1, expect=3, pipeline=3)   # forced: the heuristic is tested below
     for b in sorted({0, B // 2, B - 1}):
