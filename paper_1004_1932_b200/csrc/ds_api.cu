@@ -639,11 +639,12 @@ int setup_cluster_lat(ds_system *s) {
     if (s->pipe_mode == 0 || s->pipe_mode == 2 || s->tune_cta != 0 || s->cl_cs > 0) return DS_OK;
     if (!forced && (s->pipe_mode == 1 || s->S <= 16)) return DS_OK;
     const void *kern = cluster_lat_kernel_of(s);
-    int best_its = 1 << 30;
-    // 16 CTAs per cluster is beyond the portable size (opt-in attribute); the smallest cluster with the fewest iterations wins
-    // (S = 64: 8 CTAs 1.9 us per stage, 16 CTAs 2.0; S = 128: 2.4 / 2.2; S = 192: 3.6 / 2.7)
-    for (int cs = 2; cs <= 16; cs <<= 1) {
-        if ((long long)s->B * cs > s->num_sms || cs > s->NQ) continue;
+    double best_cost = 1e300;
+    // Cost of a stage in pair-loop iterations: waves x (iterations per warp + 4 for the tail and the hand-over); the smallest cluster
+    // wins a tie (S = 64: 4 CTAs 1.8 us per stage, 8 CTAs 1.9, 16 CTAs 2.0; S = 128: 2.4 on 8, 2.2 on 16; S = 192: 3.6 / 2.7).
+    // 16 CTAs per cluster is beyond the portable size (opt-in attribute).
+    for (int cs = 1; cs <= 16; cs <<= 1) {
+        if (cs > s->NQ || cs > s->num_sms) continue;
         const int nq = (s->NQ + cs - 1) / cs;
         if (nq > ds::CL_CW * ds::CL_MAX_QW) continue;
         int njg = 32, slots = 1, its = 0;
@@ -653,7 +654,7 @@ int setup_cluster_lat(ds_system *s) {
             const int j = (32 / QW) * m, i = (s->U + j - 1) / j;
             njg = njg > j ? njg : j; slots = slots > n * m ? slots : n * m; its = its > i ? its : i;
         }
-        if (its >= best_its || (!forced && its > LAT_MAX_ITERS)) continue;
+        if (!forced && its > LAT_MAX_ITERS) continue;
         const int buf_units = (s->U + njg + 7) / 8 * 8, rows_max = 4 * nq;
         const size_t smem = 2 * (size_t)buf_units * ds::UNIT_BYTES + 64 + (size_t)slots * 12 * 8 + (size_t)rows_max * ds::STATE_BYTES_PER_ROW;
         if (smem > (size_t)ds::SMEM_MAX) continue;
@@ -671,8 +672,16 @@ int setup_cluster_lat(ds_system *s) {
         cfg.attrs = at; cfg.numAttrs = 1;
         int n_active = 0;
         if (cudaOccupancyMaxActiveClusters(&n_active, kern, &cfg) != cudaSuccess) { (void)cudaGetLastError(); continue; }
-        if (n_active < s->B) continue;
-        best_its = its;
+        if (n_active < 1) continue;
+        const long long waves = ((long long)s->B + n_active - 1) / n_active;
+        // several waves only for one CTA per system and S > 32 (the alternatives there, run_kernel with one CTA per system or the
+        // warp-per-system kernel, run in waves too; measured: 600 x S = 64 FP32 15.3 us per stage against 22.4, but 600 x S = 20
+        // 7.8 against 3.2 of the warp-per-system kernel, and clusters of 2 or 4 in several waves lose to run_kernel: 40 x S = 100
+        // 6.5 against 5.1)
+        if (waves > 1 && !(cs == 1 && s->S > ds::SMALL_MAX_S)) continue;
+        const double cost = (double)waves * (its + 4.0);
+        if (cost >= best_cost * (1.0 - 1e-9)) continue;
+        best_cost = cost;
         s->cll_cs = cs; s->cll_buf_units = buf_units; s->cll_rows_max = rows_max; s->cll_slots_max = slots; s->cll_smem = smem;
     }
     return DS_OK;

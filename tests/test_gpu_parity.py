@@ -943,10 +943,11 @@ def test_cluster_kernel_not_taken_when_clusters_do_not_fit():
 
 # --------------------------------------------------------------------------------- small systems: a cluster of CTAs, no pipeline (cluster_lat_kernel)
 @pytest.mark.parametrize("precision,tol", [(ds.F32, 1e-4), (ds.F64, 1e-10)])
-@pytest.mark.parametrize("B,S", [(1, 17), (1, 33), (3, 40), (1, 64), (2, 99), (1, 128), (12, 128), (18, 64), (64, 40), (37, 64)])
+@pytest.mark.parametrize("B,S", [(1, 17), (1, 33), (3, 40), (1, 64), (2, 99), (1, 128), (12, 128), (18, 64), (64, 40), (37, 64), (300, 64)])
 def test_cluster_lat_kernel_shapes(B, S, precision, tol):
     """Systems with short pair loops on one cluster each (cluster_lat_kernel), the cluster size the library picks: 2 CTAs per
-    system (S = 17; the ensembles of 64 and 37), 4 (S = 33, 40, 64 = C2's shape; 18 x S = 64), 8 (12 x S = 128), 16 (S = 99, 128);
+    system (S = 17; the ensembles of 64 and 37), 4 (S = 33, 40, 64 = C2's shape; 18 x S = 64), 8 (12 x S = 128), 16 (S = 99, 128),
+    one CTA per system in three waves (300 x S = 64: 2 quads per warp);
     1 - 16 quads per CTA (16 ... 1 warps per quad, idle warps, CTAs of uneven quad counts; S = 99: a last quad of two rows).
     40 Heun steps over three calls, t0 != 0, against the oracle on every system (a sample for the big ensembles)."""
     w = inputs.config5(B=B, S=S)
@@ -983,9 +984,11 @@ def test_cluster_lat_kernel_integrators_tensors_noise_chunking(integrator, tenso
 
 def test_cluster_lat_kernel_heuristic():
     """Which shapes the library sends to cluster_lat_kernel by itself: short pair loops only (C2 yes, S = 300 no), never S <= 16
-    (warp-per-system kernel), never when the clusters are not resident at once (B = 100 x 2 CTAs)."""
+    (warp-per-system kernel), clusters of 2 or more CTAs only when all are resident at once (40 x S = 100: no), one CTA per
+    system also in waves but not for S <= 32 (600 x S = 64 yes, 600 x S = 20 no)."""
     for (B, S, precision, want) in ((1, 64, ds.F32, 3), (1, 64, ds.F64, 3), (18, 64, ds.F32, 3), (1, 20, ds.F64, 3), (1, 8, ds.F64, 0),
-                                    (1, 16, ds.F32, 0), (1, 300, ds.F64, 0), (100, 33, ds.F32, 0), (64, 256, ds.F32, 2)):
+                                    (1, 16, ds.F32, 0), (1, 300, ds.F64, 0), (100, 33, ds.F32, 3), (40, 100, ds.F32, 0),
+                                    (600, 64, ds.F32, 3), (600, 20, ds.F32, 0), (64, 256, ds.F32, 2)):
         w = inputs.config5(B=B, S=S)
         s, _ = make_system(w, precision)
         with s:
