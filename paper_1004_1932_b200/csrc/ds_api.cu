@@ -109,6 +109,8 @@ struct ds_system {
     size_t cll_smem = 0;
     size_t cl_smem = 0;
     int *half_off = nullptr;                    // device table [2][n_cta + 1]
+    int4 *ptab_g = nullptr;                     // device table [n_cta][2][16][3] (pipe_build_table)
+    size_t ptab_cap = 0;
     int half_off_cap = 0;
     int reg_units[2] = {0, 0}, pbuf_units[2] = {0, 0}, rows_max = 0;
     size_t pipe_smem = 0;
@@ -354,6 +356,19 @@ int setup_pipe(ds_system *s) {
         s->half_off_cap = 2 * (n + 1);
     }
     CU_TRY(cudaMemcpy(s->half_off, off.data(), 2 * (size_t)(n + 1) * sizeof(int), cudaMemcpyHostToDevice));
+    {   // which warp does what in the two passes of every CTA (pipe_build_table)
+        const size_t per = 2 * (size_t)ds::PIPE_CW * 3;
+        std::vector<int4> tab((size_t)n * per);
+        const int ru[2] = {off[n], off[(size_t)(n + 1) + n]};
+        for (int c = 0; c < n; ++c) ds::pipe_build_table(s->N, s->NQ, n, c, W, off.data(), ru, tab.data() + (size_t)c * per);
+        if (s->ptab_cap < tab.size()) {
+            if (s->ptab_g) CU_TRY(cudaFree(s->ptab_g));
+            s->ptab_g = nullptr; s->ptab_cap = 0;
+            CU_TRY(cudaMalloc((void **)&s->ptab_g, tab.size() * sizeof(int4)));
+            s->ptab_cap = tab.size();
+        }
+        CU_TRY(cudaMemcpy(s->ptab_g, tab.data(), tab.size() * sizeof(int4), cudaMemcpyHostToDevice));
+    }
     s->reg_units[0] = off[n]; s->reg_units[1] = off[(size_t)(n + 1) + n];
     s->pbuf_units[0] = bu[0]; s->pbuf_units[1] = bu[1];
     s->rows_max = rows_max;
@@ -380,6 +395,7 @@ int launch_pipe_run(ds_system *s, long long n_steps) {
     A.N = s->N; A.NQ = s->NQ; A.n_cta = s->n_cta; A.unit_stride = s->unit_stride;
     A.units[0] = s->units[0]; A.units[1] = s->units[1];
     A.half_off = s->half_off;
+    A.ptab_g = s->ptab_g;
     A.reg_units[0] = s->reg_units[0]; A.reg_units[1] = s->reg_units[1];
     A.buf_units[0] = s->pbuf_units[0]; A.buf_units[1] = s->pbuf_units[1];
     A.rows_max = s->rows_max;
@@ -1088,7 +1104,7 @@ int ds_destroy(ds_system *s) {
     if (!s) return DS_OK;
     cudaSetDevice(s->P.device);
     cudaStreamSynchronize(s->stream);
-    void *ptrs[] = {s->X, s->xu, s->Rref, s->msd_part, s->msd_out, s->phase, s->units[0], s->units[1], s->ll[0], s->ll[1], s->bar, s->pcnt, s->half_off, s->Xcg, s->V1g, s->Fg, s->Lg,
+    void *ptrs[] = {s->X, s->xu, s->Rref, s->msd_part, s->msd_out, s->phase, s->units[0], s->units[1], s->ll[0], s->ll[1], s->bar, s->pcnt, s->half_off, s->ptab_g, s->Xcg, s->V1g, s->Fg, s->Lg,
                     s->ap_units.p, s->st_a.p, s->st_b.p, s->st_c.p, s->avg.p, s->avg_sc.p, s->avg_xch.p};
     for (void *q : ptrs) if (q) cudaFree(q);
     (void)cudaGetLastError();

@@ -64,6 +64,7 @@ struct PipeArgs {
     unsigned long long seed;
     unsigned long long *cnt;      // [B][2] arrival counters (one per region), monotonic over launches
     unsigned long long cnt_base;
+    const int4 *ptab_g;           // device table [n_cta][2][16][3]: which warp does what in the two passes (pipe_build_table)
     long long *probe;             // dev instrumentation (DS_ENABLE_PROBE builds): PROBE_SLOTS clock samples per CTA, or NULL
 };
 
@@ -86,6 +87,67 @@ template <typename T> __device__ __forceinline__ void warp_sum12(const T (&v)[12
     for (int d = 4; d >= 1; d >>= 1) {
 #pragma unroll
         for (int i = 0; i < 3; ++i) s[i] += __shfl_xor_sync(0xffffffffu, s[i], d);
+    }
+}
+
+// Which warp does what in the two passes of CTA c (stage-invariant; built on the host once per launch shape, 9 k cycles per
+// launch when thread 0 of every CTA did it).  The 16 warps of a pass are dealt to its nqp quads, m = 16 / nqp or one more each;
+// place (quad, sub), sub < m, walks the units 32 sub + lane + k * 32 m of a region.  Entry [pass][warp] = three int4:
+// {active, quad, sub, m}, then per region {iterations of this warp, first / end of the guarded ones, slot of its sums}.
+// Places go to the four SM sub-partitions (warp % 4) so that their iteration counts balance over the whole stage;
+// sub-partition 0, which also hosts the lead service warp, gets a little less.
+inline void pipe_build_table(int N, int NQ, int n_cta, int c, int W, const int *half_off /* [2][n_cta + 1] */, const int reg_units[2],
+                             int4 *ptab /* [2][16][3] */) {
+    const int q0 = (int)((long long)c * NQ / n_cta), q1 = (int)((long long)(c + 1) * NQ / n_cta);
+    const int nq = q1 - q0;
+    const long long r0 = 4LL * q0;
+    const int nrows = (int)((N - r0) < 4 * nq ? (N - r0) : 4 * nq);
+    const int nqA = pipe_split(nq);
+    const int rowsA = 4 * nqA < nrows ? 4 * nqA : nrows, rowsB = nrows - rowsA;
+    const int ownA = half_off[c], ownB = half_off[(n_cta + 1) + c];
+    auto bounds = [&](int h, int cls, int sub, int reg) {   // the place's loop bounds
+        const int nqp = h == 0 ? nqA : nq - nqA, rows_h = h == 0 ? rowsA : rowsB;
+        const int own0 = h == 0 ? ownA : ownB, own1 = own0 + rows_h / W;
+        int4 q = make_int4(0, 0, 0, 0);
+        if (nqp > 0) {
+            const int m = PIPE_CW / nqp + cls, n_jg = 32 * m;
+            const int Ur = reg_units[reg];
+            const int its = (Ur + n_jg - 1) / n_jg;
+            // the last iteration is skipped by warps whose 32 units all lie behind the region
+            const int its_w = its - ((its > 0 && (its - 1) * n_jg + 32 * sub >= Ur) ? 1 : 0);
+            int g_lo = its_w, g_hi = its_w;     // iterations that may hold own units (alpha == beta): region h only
+            if (reg == h && rows_h > 0) {
+                g_lo = own0 / n_jg; g_hi = (own1 - 1) / n_jg + 1;
+                g_lo = g_lo < its_w ? g_lo : its_w; g_hi = g_hi < its_w ? g_hi : its_w;
+            }
+            q = make_int4(its_w, g_lo, g_hi, 0);
+        }
+        return q;
+    };
+    int load[4] = {2, 0, 0, 0};
+    for (int h = 0; h < 2; ++h) {
+        const int nqp = h == 0 ? nqA : nq - nqA;
+        int used[4] = {0, 0, 0, 0};
+        for (int w = 0; w < PIPE_CW; ++w)
+            for (int k = 0; k < 3; ++k) ptab[(h * PIPE_CW + w) * 3 + k] = make_int4(0, 0, 0, 0);
+        if (nqp == 0) continue;
+        const int mb = PIPE_CW / nqp, mr = PIPE_CW % nqp;          // quad q gets mb + (q < mr) warps
+        for (int sub = 0; sub <= mb; ++sub) {                      // heavier places (small sub) first
+            for (int quad = 0; quad < nqp; ++quad) {
+                const int cls = quad < mr ? 1 : 0, m = mb + cls;
+                if (sub >= m) continue;
+                int4 qa = bounds(h, cls, sub, 0), qb = bounds(h, cls, sub, 1);
+                const int tot = qa.x + qb.x;
+                int best = -1;
+                for (int k = 3; k >= 0; --k)   // the least loaded sub-partition with a free warp (ties: the higher one)
+                    if (used[k] < 4 && (best < 0 || load[k] < load[best])) best = k;
+                const int u = used[best]++;
+                load[best] += tot;
+                int4 *e = ptab + (h * PIPE_CW + best + 4 * u) * 3;
+                qa.w = quad * mb + (quad < mr ? quad : mr) + sub;   // slot of this place's sums in scr
+                e[0] = make_int4(1, quad, sub, m); e[1] = qa; e[2] = qb;
+            }
+        }
     }
 }
 
@@ -154,69 +216,14 @@ __global__ void __launch_bounds__(PIPE_NT, 1) pipe_kernel(const PipeArgs A) {
         }
         mbar_fence_init();
     }
-    // Which warp does what in the two passes (stage-invariant).  The 16 warps of a pass are dealt to its nqp quads, m = 16 / nqp
-    // or one more each; place (quad, sub), sub < m, walks the units 32 sub + lane + k * 32 m of a region.
-    // Step 1, one thread per (pass, m class, sub, region): the place's loop bounds (scr is free until the first pass ends).
-    int4 *const bounds = reinterpret_cast<int4 *>(scr);               // [2 passes][2 classes][16 subs][2 regions]
-    if (tid >= 64 && tid < 192) {
-        const int i = tid - 64, h = i >> 6, cls = (i >> 5) & 1, sub = (i >> 1) & 15, reg = i & 1;
-        const int nqp = h == 0 ? nqA : nq - nqA, rows_h = h == 0 ? rowsA : rowsB;
-        const int own0 = h == 0 ? ownA : ownB, own1 = own0 + rows_h / W;
-        int4 q = make_int4(0, 0, 0, 0);
-        if (nqp > 0) {
-            const int m = PIPE_CW / nqp + cls, n_jg = 32 * m;
-            const int Ur = A.reg_units[reg];
-            const int its = (Ur + n_jg - 1) / n_jg;
-            // the last iteration is skipped by warps whose 32 units all lie behind the region
-            const int its_w = its - ((its > 0 && (its - 1) * n_jg + 32 * sub >= Ur) ? 1 : 0);
-            int g_lo = its_w, g_hi = its_w;     // iterations that may hold own units (alpha == beta): region h only
-            if (reg == h && rows_h > 0) {
-                g_lo = own0 / n_jg; g_hi = (own1 - 1) / n_jg + 1;
-                g_lo = g_lo < its_w ? g_lo : its_w; g_hi = g_hi < its_w ? g_hi : its_w;
-            }
-            q = make_int4(its_w, g_lo, g_hi, 0);
-        }
-        bounds[i] = q;
-    }
+    // which warp does what in the two passes: the host's table (pipe_build_table)
+    for (int i = tid; i < 2 * PIPE_CW * 3; i += PIPE_NT) ptab[i] = A.ptab_g[(size_t)c * (2 * PIPE_CW * 3) + i];
     // far-away zero-force pad units behind each region (never overwritten: the bulk copies bring the real units only)
     for (int h = 0; h < 2; ++h) {
         uint4 *bp = reinterpret_cast<uint4 *>(h == 0 ? buf0 : buf1);
         for (int j = 3 * A.reg_units[h] + tid; j < 3 * A.buf_units[h]; j += PIPE_NT) bp[j] = pad_piece<T>(j % 3);
     }
     __syncthreads();
-    if (tid == 0) {
-        // Step 2: places go to the four SM sub-partitions (warp % 4) so that their iteration counts balance over the whole
-        // stage; sub-partition 0, which also hosts the service warp, gets a little less.
-        int load0 = 2, load1 = 0, load2 = 0, load3 = 0;
-        for (int h = 0; h < 2; ++h) {
-            const int nqp = h == 0 ? nqA : nq - nqA;
-            int used0 = 0, used1 = 0, used2 = 0, used3 = 0;
-            for (int w = 0; w < PIPE_CW; ++w) ptab[(h * PIPE_CW + w) * 3] = make_int4(0, 0, 0, 0);
-            if (nqp == 0) continue;
-            const int mb = PIPE_CW / nqp, mr = PIPE_CW % nqp;          // quad q gets mb + (q < mr) warps
-            for (int sub = 0; sub <= mb; ++sub) {                      // heavier places (small sub) first
-                for (int quad = 0; quad < nqp; ++quad) {
-                    const int cls = quad < mr ? 1 : 0, m = mb + cls;
-                    if (sub >= m) continue;
-                    int4 qa = bounds[((h * 2 + cls) * 16 + sub) * 2], qb = bounds[((h * 2 + cls) * 16 + sub) * 2 + 1];
-                    const int tot = qa.x + qb.x;
-                    int best = -1, bl = 0;
-                    if (used3 < 4) { best = 3; bl = load3; }
-                    if (used2 < 4 && (best < 0 || load2 < bl)) { best = 2; bl = load2; }
-                    if (used1 < 4 && (best < 0 || load1 < bl)) { best = 1; bl = load1; }
-                    if (used0 < 4 && (best < 0 || load0 < bl)) { best = 0; bl = load0; }
-                    int u;
-                    if (best == 3) { u = used3++; load3 += tot; }
-                    else if (best == 2) { u = used2++; load2 += tot; }
-                    else if (best == 1) { u = used1++; load1 += tot; }
-                    else { u = used0++; load0 += tot; }
-                    int4 *e = ptab + (h * PIPE_CW + best + 4 * u) * 3;
-                    qa.w = quad * mb + (quad < mr ? quad : mr) + sub;   // slot of this place's sums in scr
-                    e[0] = make_int4(1, quad, sub, m); e[1] = qa; e[2] = qb;
-                }
-            }
-        }
-    }
     {
         const double tn = time_of_step(A.t0, A.n0, A.dt);
         T *s0 = stream_of(0);
