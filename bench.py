@@ -437,9 +437,11 @@ def extras(torch, ds, inputs, w, args, precision, tensor):
                               ("C5_B64_N512_f32", inputs.config5, ds.F32, 10_000)):
         wc = w if mk is inputs.config4 else mk()
         t, _, info = time_steps(torch, ds, wc, pr, ds.RPY, nst, 64)
+        lanes_c = F64_LANES if pr == ds.F64 else F32_LANES
         cfgs[name] = {"timesteps_per_s": nst / t, "pairs_per_s": nst * 2 * pairs_per_apply(wc.N, wc.B) / t,
                       "us_per_stage": 1e6 * t / (2 * nst), "steps_per_launch": nst, "repeats": info["repeats"],
-                      "step_kernel": info["step_kernel"]}
+                      "step_kernel": info["step_kernel"],
+                      "frac_of_alu_peak": nst * 2 * pairs_per_apply(wc.N, wc.B) * FLOP_PER_PAIR["rpy"] / t / (N_SM * lanes_c * 2 * 1.965e9)}
     extra["configs_rpy_heun"] = cfgs
     extra["avg_model_eq9"] = avg_model_extra(torch, ds)
     extra["cold_l2"] = {"ms_per_step": 1e3 * time_steps_cold_l2(torch, ds, w, precision, tensor, 30),
