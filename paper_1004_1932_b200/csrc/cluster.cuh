@@ -256,7 +256,8 @@ __global__ void __launch_bounds__(CL_NT, 1) cluster_kernel(const ClusterArgs A) 
 
     if (warp < CL_CW) {
         // =========================== compute warps ===========================
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(PIPE_REGS_COMPUTE));
+        if constexpr (sizeof(T) == 8) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(PIPE_REGS_COMPUTE_F64));
+        else asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(PIPE_REGS_COMPUTE));
         const V c1 = P::bc(sizeof(T) == 4 ? (T)A.c1f : (T)A.c1), negc2 = P::bc(sizeof(T) == 4 ? (T)(-A.c2f) : (T)(-A.c2));
         for (int g = 0; g < n_stage; ++g) {
             const int par = g & 1;
@@ -315,7 +316,9 @@ __global__ void __launch_bounds__(CL_NT, 1) cluster_kernel(const ClusterArgs A) 
             }
         }
     } else {
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(PIPE_REGS_SERVICE));   // all four warps of the service warpgroup
+        // all four warps of the service warpgroup
+        if constexpr (sizeof(T) == 8) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(PIPE_REGS_SERVICE_F64));
+        else asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(PIPE_REGS_SERVICE));
     }
     if (warp >= CL_CW) {
         // =========================== service warpgroup ===========================
